@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the PGG Monte Carlo sweep on BASELINE.json configs[4].
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--fmt u8|bits] [--L 16384] [--mcs 1000] [--variant auto|v0|tile]
+
+One *step* is one whole pass of the hot path over the throughput workload: Bernoulli(0.5)
+initial condition from seed 1 (K0) followed by `--mcs` full Monte Carlo steps (16 phase
+launches each: class draw, staging, Philox draws, payoff differences, acceptance,
+in-place writes, fused density) on a single L x L lattice, r = 3.8, K = 0.5.
+Metric: elementary strategy updates per second (BASELINE.json `metric`), plus the
+fraction of the HBM roofline for the sweep's contract bytes (17 B/update for uint8,
+SURVEY.md section 8(d)).
+
+N > 1 (torchrun): the path has no exchange step on one GPU, so ranks run independent
+replicas (rank q uses seed 1+q) -- weak scaling, no data-path collective.
+
+`--impl reference` times the CPU oracle (oracle/, plain C, as it stands) on the host
+cores, one MCS of the same workload per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+R, K_NOISE, RHO0, SEED = 3.8, 0.5, 0.5, 1           # BASELINE.json configs[4]
+METRIC = "elementary strategy updates/sec at L=16384"
+
+
+def load_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown",
+                                "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(L: int, max_mcs: int, min_seconds: float):
+    """Time the oracle (as it stands) on `max_mcs` MCS of the workload, all host threads."""
+    import numpy as np
+    import oracle as orc
+    threads = orc.max_threads()
+    lat = orc.init(L, RHO0, SEED)
+    done, t0 = 0, time.perf_counter()
+    while done < max_mcs:
+        orc.sweep(lat, R, K_NOISE, SEED, orc.ORDER_IID, done, 1, n_threads=threads)
+        done += 1
+        if time.perf_counter() - t0 >= min_seconds:
+            break
+    dt = time.perf_counter() - t0
+    return done * L * L / dt, threads, done, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as orc
+    L = args.L
+    threads = orc.max_threads()
+    lat = orc.init(L, RHO0, SEED)
+    t = 0
+    for _ in range(args.warmup):
+        orc.sweep(lat, R, K_NOISE, SEED, orc.ORDER_IID, t, 1, n_threads=threads); t += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.sweep(lat, R, K_NOISE, SEED, orc.ORDER_IID, t, 1, n_threads=threads); t += 1
+    dt = time.perf_counter() - t0
+    value = args.steps * L * L / dt
+    sample = (f"each step = 1 MCS (MCS {args.warmup}..{t - 1}) of the L={L} workload from the "
+              f"Bernoulli(0.5) seed-1 start; oracle/pgg_oracle.c -O2, rows of a class split over threads")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "updates/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+        "data": "synthetic", "config": {"workload": f"C5 L={L} r={R} K={K_NOISE} rho0={RHO0} seed={SEED}",
+                                        "fmt": "u8", "mcs_per_step": 1},
+        "cpu_baseline": {"value": value, "unit": "updates/s", "cores": threads, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1704_08098_b200 as pgg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    pgg.lib()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    L, n_mcs = args.L, args.mcs
+    fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
+    variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
+               "fused": pgg.VARIANT_FUSED}[args.variant]
+    pgg.pgg_set_variant(variant)
+    seed = SEED + rank
+    shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
+    tdtype = torch.uint8 if fmt == pgg.FMT_U8 else torch.int32
+    d_lat = torch.empty(shape, dtype=tdtype, device="cuda")
+    d_counts = torch.zeros(n_mcs, dtype=torch.int64, device="cuda")
+    stream = torch.cuda.current_stream()
+    lat_bytes = d_lat.numel() * d_lat.element_size()
+
+    ev_a = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev_b = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev_c = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+
+    def step(i=None):
+        if i is not None:
+            ev_a[i].record(stream)
+        pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
+        if i is not None:
+            ev_b[i].record(stream)
+        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, n_mcs, d_counts, stream)
+        if i is not None:
+            ev_c[i].record(stream)
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = pgg.pgg_launch_count()
+    for i in range(args.steps):
+        step(i)
+    barrier()
+    launches = pgg.pgg_launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev_a[0].elapsed_time(ev_c[-1])
+    sweep_ms = sum(ev_b[i].elapsed_time(ev_c[i]) for i in range(args.steps))
+    last_counts = d_counts.cpu()
+    if world > 1:
+        t = torch.tensor([total_ms, sweep_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, sweep_ms = t.tolist()
+    updates_per_step = float(n_mcs) * L * L
+    value = world * args.steps * updates_per_step / (total_ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): per step copy the initial
+    # lattice host->device, sweep, copy the final lattice and the count trace device->host.
+    h_lat0 = torch.empty(shape, dtype=tdtype).pin_memory()
+    pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
+    h_lat0.copy_(d_lat)
+    h_out = torch.empty(shape, dtype=tdtype).pin_memory()
+    h_counts = torch.empty(n_mcs, dtype=torch.int64).pin_memory()
+
+    def e2e_step():
+        d_lat.copy_(h_lat0, non_blocking=True)
+        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, n_mcs, d_counts, stream)
+        h_out.copy_(d_lat, non_blocking=True)
+        h_counts.copy_(d_counts, non_blocking=True)
+        stream.synchronize()
+
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    e2e_ms = max(e0.elapsed_time(e1), 0.0)
+    e2e_wall_ms = (time.perf_counter() - t0) * 1e3
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = t.item()
+    e2e_value = world * e2e_steps * updates_per_step / (e2e_ms * 1e-3)
+    assert torch.equal(h_counts, last_counts), "e2e run and device-resident run disagree"
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the phase kernel; 16 launches per MCS)
+    peak, peak_src = load_peaks()
+    n_phase = 16 * n_mcs * args.steps
+    phase_us = sweep_ms * 1e3 / n_phase            # includes the per-call order/density/finalize kernels
+    b_site = 1.0 if fmt == pgg.FMT_U8 else 0.125
+    bytes_per_launch = (L * L + L * L / 16.0) * b_site   # read the lattice, write the active class
+    achieved = bytes_per_launch / (phase_us * 1e-6) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "kernel": "phase kernel (variant %d)" % pgg.pgg_get_variant_used(),
+                "avg_launch_us": phase_us, "algorithmic_bytes_per_launch": bytes_per_launch,
+                "note": "17 B/update contract bytes (16 phases x (read N + write N/16)), SURVEY 8(d)"
+                        + ("; the 32 MiB packed lattice is L2-resident, so this is not a DRAM fraction"
+                           if fmt == pgg.FMT_BITS else "")}
+    tr = ROOT / "profiles" / "traffic.json"
+    if tr.exists():
+        try:
+            roofline["traffic"] = json.loads(tr.read_text()).get(f"{args.fmt}_L{L}_bytes_per_launch")
+        except (ValueError, OSError):
+            pass
+
+    out = {
+        "metric": METRIC, "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u8" if fmt == pgg.FMT_U8 else "u1 (bit-packed u32)",
+        "data": "synthetic",
+        "config": {"workload": f"C5 throughput: single L={L} lattice, Bernoulli(0.5) init seed 1, r={R}, "
+                               f"K={K_NOISE}, {n_mcs} MCS per step (init + sweep + fused rho_C trace)",
+                   "fmt": args.fmt, "L": L, "mcs_per_step": n_mcs, "order_mode": "iid",
+                   "variant": pgg.pgg_get_variant_used(),
+                   "l2": ("inputs larger than L2 (256 MiB lattice re-read every phase)" if lat_bytes > 130e6
+                          else "lattice fits L2 by nature of the workload; no flush"),
+                   "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+        "mcs_per_s": world * args.steps * n_mcs / (total_ms * 1e-3),
+        "sweep_only_updates_per_s": args.steps * updates_per_step / (sweep_ms * 1e-3),
+        "final_rho_C": float(last_counts[-1]) / (L * L),
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "updates/s", "h2d_bytes_per_step": lat_bytes,
+                "d2h_bytes_per_step": lat_bytes + 8 * n_mcs, "steps": e2e_steps,
+                "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": e2e_wall_ms / e2e_steps},
+        "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        v, threads, n_done, dt = oracle_sample(L, max_mcs=8, min_seconds=10.0)
+        out["cpu_baseline"] = {"value": v, "unit": "updates/s", "cores": threads, "kind": "oracle",
+                               "sample": f"first {n_done} MCS of the same L={L} workload ({dt:.1f} s wall), "
+                                         f"oracle/pgg_oracle.c as it stands, class rows split over "
+                                         f"{threads} OpenMP threads"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
+    ap.add_argument("--L", type=int, default=16384)
+    ap.add_argument("--mcs", type=int, default=1000)
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,146 @@
+/*
+ * pgg.h -- C ABI of libpgg: the Monte Carlo sweep of the spatial public goods
+ * game (Perc, arXiv:1704.08098) on an L x L periodic square lattice, run under
+ * the race-free 16-sublattice Philox schedule, as hand-written CUDA for sm_100a.
+ *
+ * Citations are "PAPER.md:<line>" (the paper's text, /root/reference/PAPER.md)
+ * and "SURVEY 8(c) Dn/Sn" (the readings listed in SURVEY.md section 8(c) and
+ * restated in DESIGN.md).  Everything the method computes runs in CUDA kernels
+ * of this library; there is no CPU fallback.  Every entry point returns
+ * PGG_OK (0) or a negative PGG_ERR_* code; nothing is printed, no exception
+ * crosses the boundary.  pgg_last_error() gives a thread-local text.
+ *
+ * Model.  s(i,j) in {0,1}: D = 0, C = 1.  cross(z) = z and its
+ * four nearest neighbours (the von Neumann group centred on z, G = 5).
+ * N(z) = number of cooperators in cross(z).  A_x = sum of N(z) over the five
+ * groups z in cross(x) that player x belongs to.  With c = 1 (Eqs. 1-2,
+ * PAPER.md:47-50) the total payoff is  Pi_x = (r/5) A_x - 5 s_x.
+ * Elementary step: focal x, random nearest neighbour y, x adopts
+ * s_y with W = 1/(1+exp((Pi_x-Pi_y)/K))  (Eq. 3).
+ *
+ * Schedule (north_star).  class(i,j) = 4*(i mod 4) +
+ * (j mod 4).  One MCS t = 16 phases k = 0..15; phase k updates, in place and
+ * all at once, every site of one class c(t,k) drawn from Philox4x32-10; each
+ * site draws (direction, u) from Philox4x32-10 with counter
+ * (site, t, (k<<8)|c, 3) and key (seed lo, seed hi); x adopts s_y iff
+ * s_x != s_y and u < T[(s_x-s_y+1)*51 + (A_x-A_y+25)].
+ *
+ * Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller
+ * owns every buffer.  `stream` is a cudaStream_t passed as void* (NULL = the
+ * legacy default stream).  All device work is enqueued on `stream`; no entry
+ * point synchronises with the host, results are valid once the caller has
+ * synchronised the stream.  Temporary device memory is taken and returned
+ * with the stream-ordered allocator (cudaMallocAsync / cudaFreeAsync).
+ */
+#ifndef PGG_H_
+#define PGG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    PGG_OK = 0,
+    PGG_ERR_NULL = -1,        /* a required pointer is NULL                              */
+    PGG_ERR_BAD_L = -2,       /* L < 4, L % 4 != 0, L > 65536, or (bits) L % 32 != 0     */
+    PGG_ERR_BAD_PARAM = -3,   /* r/K not finite, K <= 0, rho0 outside [0,1], B == 0, ... */
+    PGG_ERR_ALIGN = -4,       /* lattice pointer not 16-byte aligned                     */
+    PGG_ERR_UNSUPPORTED = -5, /* unknown fmt / order_mode / kernel variant               */
+    PGG_ERR_CUDA = -6         /* a CUDA runtime call failed; see pgg_last_error()        */
+};
+
+/* Canonical lattice layouts.
+ * PGG_FMT_U8  : row-major uint8 [L][L], 1 = C, 0 = D.  Any L with L % 4 == 0.
+ * PGG_FMT_BITS: row-major, site (i,j) is bit (j & 31) of the little-endian uint32
+ *               word i*(L/32) + (j >> 5).  Needs L % 32 == 0.                    */
+enum { PGG_FMT_U8 = 0, PGG_FMT_BITS = 1 };
+
+/* How the 16 phase classes of an MCS are drawn.
+ * PGG_ORDER_IID : class of phase k = top 4 bits of word k (default; reproduces
+ *                 random-sequential statistics).
+ * PGG_ORDER_PERM: a permutation -- classes sorted by (word[c], c).               */
+enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1 };
+
+/* Kernel variants of the phase step (all bit-identical).
+ * PGG_VARIANT_AUTO picks the fastest one that supports (fmt, L).                 */
+enum {
+    PGG_VARIANT_AUTO = 0,
+    PGG_VARIANT_V0 = 1,   /* one thread per active site, global loads, any L % 4 == 0 */
+    PGG_VARIANT_TILE = 2, /* smem tile + 3-site halo, bulk-async staged, compaction   */
+    PGG_VARIANT_FUSED = 3 /* several phases per tile residency (temporal blocking)    */
+};
+
+/* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:
+ * for ds in {-1,0,1}, dA in [-25,25], in IEEE double and in this order,
+ *   delta = (r*dA)/5 - 5*ds;  W = 1/(1+exp(delta/K));  v = W * 2^32;
+ *   T = v >= 4294967295 ? 0xFFFFFFFF : (uint32)floor(v)
+ * stored at out153[(ds+1)*51 + (dA+25)].  Pure host function (no CUDA call).
+ * h_out153: host array of 153 uint32, written.
+ * Errors: NULL -> PGG_ERR_NULL; r or K not finite, K <= 0 -> PGG_ERR_BAD_PARAM. */
+int32_t pgg_build_accept_table(double r, double K, uint32_t* h_out153);
+
+/* Initial condition ("C or D with equal probability"):
+ * s(site) = [ x0 < floor(rho0 * 2^32) ], (x0,..) = Philox4x32-10(ctr = (site,0,0,1),
+ * key = seed).  rho0 = 0 gives all D, rho0 = 1 all C, exactly.
+ * d_lat: device lattice in layout `fmt`, L*L bytes (u8) or L*L/8 bytes (bits),
+ * 16-byte aligned, overwritten.                                                  */
+int32_t pgg_init_lattice(void* d_lat, int32_t fmt, uint32_t L, double rho0, uint64_t seed,
+                         void* stream);
+
+/* n_mcs full Monte Carlo steps t = t_begin .. t_begin+n_mcs-1 (1 MCS = L^2
+ * elementary steps, PAPER.md:65 = 16 phases of L^2/16 sites), in place.
+ * d_counts: NULL, or device array of n_mcs uint64; d_counts[m] = number of
+ *   cooperators (numerator of Eq. 4) after MCS t_begin+m completes.
+ * The RNG is counter based, so (t_begin=a, n=b) followed by (a+b, c) equals
+ * (a, b+c) bit for bit.
+ * Errors: PGG_ERR_NULL (d_lat), PGG_ERR_BAD_L, PGG_ERR_ALIGN, PGG_ERR_BAD_PARAM
+ * (r, K not finite, K <= 0, t_begin + n_mcs > 2^32), PGG_ERR_UNSUPPORTED
+ * (fmt, order_mode), PGG_ERR_CUDA.  n_mcs == 0 is a no-op.                        */
+int32_t pgg_sweep(void* d_lat, int32_t fmt, uint32_t L, double r, double K, uint64_t seed,
+                  int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
+                  void* stream);
+
+/* Cooperator count sum_x d_x (Eq. 4; rho_C = count / L^2).
+ * d_count: device uint64, overwritten.                                           */
+int32_t pgg_density(const void* d_lat, int32_t fmt, uint32_t L, uint64_t* d_count, void* stream);
+
+/* B independent lattices in one grid per phase (north_star (5)): lattice b has
+ * its own r (h_r[b]) and seed (h_seeds[b]) and therefore its own acceptance
+ * table, phase-class order and draws; it evolves exactly as a solo pgg_sweep
+ * with (h_r[b], h_seeds[b]) would.
+ * d_lats : B lattices, contiguous, each L*L bytes (u8) or L*L/8 bytes (bits).
+ * h_r, h_seeds: host arrays of B entries, read before the call returns.
+ * rho0   : in [0,1] -> first initialise lattice b by pgg_init_lattice(seed b);
+ *          < 0 -> continue from the state given in d_lats.
+ * d_counts: NULL or device array [B][n_mcs] uint64, as in pgg_sweep.             */
+int32_t pgg_run_ensemble(void* d_lats, int32_t fmt, uint32_t B, uint32_t L, const double* h_r,
+                         double K, const uint64_t* h_seeds, int32_t order_mode, double rho0,
+                         uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts, void* stream);
+
+/* The 16 phase classes of MCS t, computed by the library's own
+ * device kernel and copied back; h_out16: host array of 16 bytes.  Synchronises
+ * `stream`.  For tests of step a1.                                               */
+int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t* h_out16,
+                          void* stream);
+
+/* Select the phase-kernel variant used by pgg_sweep / pgg_run_ensemble from now
+ * on (process-wide; PGG_VARIANT_*).  Returns PGG_ERR_UNSUPPORTED if unknown.
+ * pgg_get_variant_used() reports the variant the last sweep on this thread ran. */
+int32_t pgg_set_variant(int32_t variant);
+int32_t pgg_get_variant_used(void);
+
+/* 1 if kernel variant `variant` can run lattices of layout fmt and size L, else 0. */
+int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L);
+
+/* Number of kernels this library has launched in this process (monotone).       */
+uint64_t pgg_launch_count(void);
+
+/* Text of the last error on the calling thread ("" if none).                    */
+const char* pgg_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PGG_H_ */

@@ -1,0 +1,342 @@
+// pgg.cu -- the C ABI of libpgg (include/pgg.h): argument validation, the host
+// acceptance-table builder, stream-ordered temporaries and the launch sequence
+// of a sweep.  Every step of the method itself runs in the CUDA kernels.
+// Compile: nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo (see build.py).
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/pgg.h"
+#include "pgg_common.cuh"
+#include "pgg_kernels_v0.cuh"
+#include "pgg_kernels_tile.cuh"
+
+namespace {
+
+thread_local std::string g_last_error;
+thread_local int g_variant_used = PGG_VARIANT_AUTO;
+std::atomic<int> g_variant{PGG_VARIANT_AUTO};
+std::atomic<unsigned long long> g_launches{0};
+
+int32_t fail(int32_t code, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_last_error = buf;
+    return code;
+}
+
+#define PGG_CUDA(call)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(PGG_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),  \
+                        __FILE__, __LINE__);                                                   \
+    } while (0)
+
+#define PGG_LAUNCHED()                                                                         \
+    do {                                                                                       \
+        g_launches.fetch_add(1, std::memory_order_relaxed);                                    \
+        PGG_CUDA(cudaGetLastError());                                                          \
+    } while (0)
+
+int32_t check_lattice_args(const void* d_lat, int32_t fmt, uint32_t L)
+{
+    if (d_lat == nullptr) return fail(PGG_ERR_NULL, "lattice pointer is NULL");
+    if (fmt != PGG_FMT_U8 && fmt != PGG_FMT_BITS) return fail(PGG_ERR_UNSUPPORTED, "unknown fmt %d", fmt);
+    if (L < 4 || L % 4 != 0 || L > 65536)
+        return fail(PGG_ERR_BAD_L, "L = %u: need 4 <= L <= 65536 and L %% 4 == 0", L);
+    if (fmt == PGG_FMT_BITS && L % 32 != 0)
+        return fail(PGG_ERR_BAD_L, "L = %u: the bit-packed layout needs L %% 32 == 0", L);
+    if ((reinterpret_cast<uintptr_t>(d_lat) & 15u) != 0)
+        return fail(PGG_ERR_ALIGN, "lattice pointer must be 16-byte aligned");
+    return PGG_OK;
+}
+
+inline unsigned long long lattice_bytes(int32_t fmt, uint32_t L)
+{
+    const unsigned long long n = (unsigned long long)L * L;
+    return fmt == PGG_FMT_U8 ? n : n / 8;
+}
+
+// Device temporaries of one call, returned to the stream-ordered pool on scope exit.
+struct Scratch {
+    cudaStream_t stream;
+    std::vector<void*> ptrs;
+    explicit Scratch(cudaStream_t s) : stream(s) {}
+    ~Scratch()
+    {
+        for (void* p : ptrs) cudaFreeAsync(p, stream);
+    }
+    cudaError_t alloc(void** p, size_t bytes)
+    {
+        cudaError_t e = cudaMallocAsync(p, bytes ? bytes : 16, stream);
+        if (e == cudaSuccess) ptrs.push_back(*p);
+        return e;
+    }
+};
+
+int32_t launch_init(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, double rho0,
+                    const uint64_t* d_seeds, cudaStream_t stream)
+{
+    // thr = floor(rho0 * 2^32) in [0, 2^32]  (D4)
+    const unsigned long long thr = (unsigned long long)std::floor(rho0 * 4294967296.0);
+    const uint32_t n_sites = L * L;  // L <= 65536: L*L may be 2^32 -> handled below
+    if (L == 65536) return fail(PGG_ERR_BAD_L, "L = 65536: site index does not fit the init counter");
+    const unsigned long long lb = lattice_bytes(fmt, L);
+    const uint32_t n_items = fmt == PGG_FMT_U8 ? n_sites >> 4 : n_sites >> 5;
+    uint32_t gx = (n_items + 255) / 256;
+    if (gx == 0) gx = 1;
+    if (gx > 148u * 64u) gx = 148u * 64u;
+    dim3 grid(gx, B);
+    if (fmt == PGG_FMT_U8)
+        pgg::init_u8_kernel<<<grid, 256, 0, stream>>>(d_lats, lb, d_seeds, n_sites, thr);
+    else
+        pgg::init_bits_kernel<<<grid, 256, 0, stream>>>(d_lats, lb, d_seeds, n_sites, thr);
+    PGG_LAUNCHED();
+    return PGG_OK;
+}
+
+int32_t launch_density(const uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L,
+                       unsigned long long* d_out, uint32_t out_stride, cudaStream_t stream)
+{
+    const unsigned long long lb = lattice_bytes(fmt, L);
+    unsigned long long n16 = lb >> 4;
+    uint32_t gx = (uint32_t)std::min<unsigned long long>((n16 + 1023) / 1024, 148ull * 16ull);
+    if (gx == 0) gx = 1;
+    dim3 grid(gx, B);
+    if (fmt == PGG_FMT_U8)
+        pgg::density_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(d_lats, lb, d_out, out_stride);
+    else
+        pgg::density_kernel<pgg::kFmtBits><<<grid, 256, 0, stream>>>(d_lats, lb, d_out, out_stride);
+    PGG_LAUNCHED();
+    return PGG_OK;
+}
+
+// The sweep proper for B lattices (B = 1: pgg_sweep).
+int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const double* h_r, double K,
+                   const uint64_t* h_seeds, int32_t order_mode, double rho0, uint32_t t_begin,
+                   uint32_t n_mcs, uint64_t* d_counts, cudaStream_t stream)
+{
+    if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM)
+        return fail(PGG_ERR_UNSUPPORTED, "unknown order_mode %d", order_mode);
+    if (!(K > 0.0) || !std::isfinite(K)) return fail(PGG_ERR_BAD_PARAM, "K must be finite and > 0");
+    for (uint32_t b = 0; b < B; ++b)
+        if (!std::isfinite(h_r[b])) return fail(PGG_ERR_BAD_PARAM, "r[%u] is not finite", b);
+    if ((unsigned long long)t_begin + n_mcs > 4294967296ull)
+        return fail(PGG_ERR_BAD_PARAM, "t_begin + n_mcs exceeds 2^32");
+    if (L == 65536) return fail(PGG_ERR_BAD_L, "L = 65536: site index does not fit uint32 counters");
+
+    int variant = g_variant.load();
+    const bool tile_ok = pgg::tile_supported(fmt, L);
+    if (variant == PGG_VARIANT_AUTO) variant = tile_ok ? PGG_VARIANT_TILE : PGG_VARIANT_V0;
+    if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_FUSED) && !tile_ok)
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
+    if (variant == PGG_VARIANT_FUSED) return fail(PGG_ERR_UNSUPPORTED, "fused variant not built");
+    g_variant_used = variant;
+
+    Scratch tmp(stream);
+    // per-lattice seeds and acceptance tables
+    std::vector<uint32_t> h_tables((size_t)B * pgg::kTableSize);
+    for (uint32_t b = 0; b < B; ++b) {
+        int32_t rc = pgg_build_accept_table(h_r[b], K, h_tables.data() + (size_t)b * pgg::kTableSize);
+        if (rc != PGG_OK) return rc;
+    }
+    uint64_t* d_seeds = nullptr;
+    uint32_t* d_tables = nullptr;
+    PGG_CUDA(tmp.alloc((void**)&d_seeds, sizeof(uint64_t) * B));
+    PGG_CUDA(tmp.alloc((void**)&d_tables, sizeof(uint32_t) * h_tables.size()));
+    // pageable sources: the runtime stages them before returning, so the host
+    // vectors may die at scope exit
+    PGG_CUDA(cudaMemcpyAsync(d_seeds, h_seeds, sizeof(uint64_t) * B, cudaMemcpyHostToDevice, stream));
+    PGG_CUDA(cudaMemcpyAsync(d_tables, h_tables.data(), sizeof(uint32_t) * h_tables.size(),
+                             cudaMemcpyHostToDevice, stream));
+
+    if (rho0 >= 0.0) {
+        int32_t rc = launch_init(d_lats, fmt, B, L, rho0, d_seeds, stream);
+        if (rc != PGG_OK) return rc;
+    }
+    if (n_mcs == 0) return PGG_OK;
+
+    unsigned long long* d_count0 = nullptr;
+    if (d_counts != nullptr) {
+        PGG_CUDA(tmp.alloc((void**)&d_count0, sizeof(unsigned long long) * B));
+        PGG_CUDA(cudaMemsetAsync(d_count0, 0, sizeof(unsigned long long) * B, stream));
+        PGG_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(uint64_t) * (size_t)B * n_mcs, stream));
+        int32_t rc = launch_density(d_lats, fmt, B, L, d_count0, 1, stream);
+        if (rc != PGG_OK) return rc;
+    }
+
+    const uint32_t chunk = std::min<uint32_t>(n_mcs, 4096u);
+    uint8_t* d_order = nullptr;
+    PGG_CUDA(tmp.alloc((void**)&d_order, (size_t)B * chunk * 16));
+
+    pgg::PhaseArgs a;
+    a.lats = d_lats;
+    a.lat_bytes = lattice_bytes(fmt, L);
+    a.seeds = d_seeds;
+    a.tables = d_tables;
+    a.order = d_order;
+    a.deltas = reinterpret_cast<unsigned long long*>(d_counts);
+    a.L = L;
+    a.order_stride = chunk;
+    a.n_mcs = n_mcs;
+    a.t_begin = t_begin;
+
+    pgg::TilePlan plan;
+    if (variant == PGG_VARIANT_TILE) {
+        int32_t rc = pgg::tile_plan(fmt, L, B, &plan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "tile kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
+
+    for (uint32_t m0 = 0; m0 < n_mcs; m0 += chunk) {
+        const uint32_t n_chunk = std::min<uint32_t>(chunk, n_mcs - m0);
+        pgg::order_kernel<<<(B * n_chunk + 127) / 128, 128, 0, stream>>>(
+            d_seeds, B, t_begin + m0, n_chunk, chunk, order_mode, d_order);
+        PGG_LAUNCHED();
+        for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
+            for (uint32_t k = 0; k < 16; ++k) {
+                if (variant == PGG_VARIANT_TILE) {
+                    pgg::tile_launch(plan, fmt, a, m, k, stream);
+                } else {
+                    const uint32_t n_cls = (L / 4) * (L / 4);
+                    dim3 grid((n_cls + 255) / 256, B);
+                    if (fmt == PGG_FMT_U8)
+                        pgg::phase_v0_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, m, k);
+                    else
+                        pgg::phase_v0_kernel<pgg::kFmtBits><<<grid, 256, 0, stream>>>(a, m, k);
+                }
+                PGG_LAUNCHED();
+            }
+        }
+    }
+    if (d_counts != nullptr) {
+        pgg::finalize_counts_kernel<<<B, 1024, 0, stream>>>(
+            reinterpret_cast<unsigned long long*>(d_counts), n_mcs, d_count0);
+        PGG_LAUNCHED();
+    }
+    return PGG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t pgg_build_accept_table(double r, double K, uint32_t* h_out153)
+{
+    if (h_out153 == nullptr) return fail(PGG_ERR_NULL, "out153 is NULL");
+    if (!std::isfinite(r) || !std::isfinite(K) || !(K > 0.0))
+        return fail(PGG_ERR_BAD_PARAM, "r and K must be finite, K > 0");
+    // Eq. (3), in the operation order of SURVEY 8(c) D3.  Pi_x - Pi_y =
+    // (r/5)(A_x - A_y) - 5 (s_x - s_y) because Pi = (r/5) A - 5 s (c = 1).
+    for (int ds = -1; ds <= 1; ++ds) {
+        for (int dA = -25; dA <= 25; ++dA) {
+            volatile double delta = (r * (double)dA) / 5.0 - 5.0 * (double)ds;
+            volatile double z = delta / K;
+            volatile double W = 1.0 / (1.0 + std::exp(z));
+            const double v = W * 4294967296.0;
+            h_out153[(ds + 1) * 51 + (dA + 25)] =
+                (v >= 4294967295.0) ? 0xFFFFFFFFu : (uint32_t)std::floor(v);
+        }
+    }
+    return PGG_OK;
+}
+
+int32_t pgg_init_lattice(void* d_lat, int32_t fmt, uint32_t L, double rho0, uint64_t seed, void* stream)
+{
+    int32_t rc = check_lattice_args(d_lat, fmt, L);
+    if (rc != PGG_OK) return rc;
+    if (!(rho0 >= 0.0 && rho0 <= 1.0)) return fail(PGG_ERR_BAD_PARAM, "rho0 must lie in [0,1]");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    Scratch tmp(s);
+    uint64_t* d_seed = nullptr;
+    PGG_CUDA(tmp.alloc((void**)&d_seed, sizeof(uint64_t)));
+    PGG_CUDA(cudaMemcpyAsync(d_seed, &seed, sizeof seed, cudaMemcpyHostToDevice, s));
+    return launch_init(static_cast<uint8_t*>(d_lat), fmt, 1, L, rho0, d_seed, s);
+}
+
+int32_t pgg_sweep(void* d_lat, int32_t fmt, uint32_t L, double r, double K, uint64_t seed,
+                  int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts, void* stream)
+{
+    int32_t rc = check_lattice_args(d_lat, fmt, L);
+    if (rc != PGG_OK) return rc;
+    return run_sweeps(static_cast<uint8_t*>(d_lat), fmt, 1, L, &r, K, &seed, order_mode, -1.0, t_begin,
+                      n_mcs, d_counts, static_cast<cudaStream_t>(stream));
+}
+
+int32_t pgg_density(const void* d_lat, int32_t fmt, uint32_t L, uint64_t* d_count, void* stream)
+{
+    int32_t rc = check_lattice_args(d_lat, fmt, L);
+    if (rc != PGG_OK) return rc;
+    if (d_count == nullptr) return fail(PGG_ERR_NULL, "d_count is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    PGG_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint64_t), s));
+    return launch_density(static_cast<const uint8_t*>(d_lat), fmt, 1, L,
+                          reinterpret_cast<unsigned long long*>(d_count), 1, s);
+}
+
+int32_t pgg_run_ensemble(void* d_lats, int32_t fmt, uint32_t B, uint32_t L, const double* h_r, double K,
+                         const uint64_t* h_seeds, int32_t order_mode, double rho0, uint32_t t_begin,
+                         uint32_t n_mcs, uint64_t* d_counts, void* stream)
+{
+    int32_t rc = check_lattice_args(d_lats, fmt, L);
+    if (rc != PGG_OK) return rc;
+    if (h_r == nullptr || h_seeds == nullptr) return fail(PGG_ERR_NULL, "h_r / h_seeds is NULL");
+    if (B == 0 || B > 65535) return fail(PGG_ERR_BAD_PARAM, "B = %u: need 1 <= B <= 65535", B);
+    if (rho0 > 1.0 || rho0 != rho0) return fail(PGG_ERR_BAD_PARAM, "rho0 must be <= 1 (or < 0 to continue)");
+    return run_sweeps(static_cast<uint8_t*>(d_lats), fmt, B, L, h_r, K, h_seeds, order_mode, rho0,
+                      t_begin, n_mcs, d_counts, static_cast<cudaStream_t>(stream));
+}
+
+int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t* h_out16, void* stream)
+{
+    if (h_out16 == nullptr) return fail(PGG_ERR_NULL, "h_out16 is NULL");
+    if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM)
+        return fail(PGG_ERR_UNSUPPORTED, "unknown order_mode %d", order_mode);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    Scratch tmp(s);
+    uint64_t* d_seed = nullptr;
+    uint8_t* d_order = nullptr;
+    PGG_CUDA(tmp.alloc((void**)&d_seed, sizeof(uint64_t)));
+    PGG_CUDA(tmp.alloc((void**)&d_order, 16));
+    PGG_CUDA(cudaMemcpyAsync(d_seed, &seed, sizeof seed, cudaMemcpyHostToDevice, s));
+    pgg::order_kernel<<<1, 128, 0, s>>>(d_seed, 1, t, 1, 1, order_mode, d_order);
+    PGG_LAUNCHED();
+    PGG_CUDA(cudaMemcpyAsync(h_out16, d_order, 16, cudaMemcpyDeviceToHost, s));
+    PGG_CUDA(cudaStreamSynchronize(s));
+    return PGG_OK;
+}
+
+int32_t pgg_set_variant(int32_t variant)
+{
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_FUSED)
+        return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
+    g_variant.store(variant);
+    return PGG_OK;
+}
+
+int32_t pgg_get_variant_used(void) { return g_variant_used; }
+
+int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
+{
+    if (fmt != PGG_FMT_U8 && fmt != PGG_FMT_BITS) return 0;
+    if (L < 4 || L % 4 != 0 || L >= 65536 || (fmt == PGG_FMT_BITS && L % 32 != 0)) return 0;
+    if (variant == PGG_VARIANT_AUTO || variant == PGG_VARIANT_V0) return 1;
+    if (variant == PGG_VARIANT_TILE) return pgg::tile_supported(fmt, L) ? 1 : 0;
+    return 0;
+}
+
+uint64_t pgg_launch_count(void) { return g_launches.load(); }
+
+const char* pgg_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,329 @@
+"""GPU <-> oracle parity, bit for bit, through the C ABI (``-m gpu``).
+
+Every case runs the same seeded input through ``libpgg`` (CUDA, sm_100a) and
+through ``oracle/`` (plain C on the CPU) and compares every lattice site and
+every cooperator count.  Integer work: the bar is exact equality."""
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+import paper_1704_08098_b200 as pgg  # noqa: E402
+
+K = wl.K_DEFAULT
+FMTS = [pgg.FMT_U8, pgg.FMT_BITS]
+VARIANTS = [pgg.VARIANT_V0, pgg.VARIANT_TILE]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (there is no CPU fallback)")
+    pgg.lib()
+    yield
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+
+
+def use_variant(v, fmt, L):
+    """Select kernel variant v; skip if it does not support (fmt, L)."""
+    if not pgg.pgg_variant_supported(v, fmt, L):
+        pytest.skip("this variant does not support this (fmt, L)")
+    pgg.pgg_set_variant(v)
+
+
+# ---------------------------------------------------------------- marshalling helpers
+def to_device(lat, fmt):
+    """numpy uint8 [.., L, L] -> device tensor in layout fmt (packing is pure layout)."""
+    lat = np.ascontiguousarray(lat, dtype=np.uint8)
+    if fmt == pgg.FMT_U8:
+        return torch.from_numpy(lat).cuda()
+    L = lat.shape[-1]
+    bits = lat.reshape(lat.shape[:-1] + (L // 32, 32)).astype(np.uint32)
+    words = (bits << np.arange(32, dtype=np.uint32)).sum(axis=-1, dtype=np.uint64).astype(np.uint32)
+    return torch.from_numpy(words.view(np.int32)).cuda()
+
+
+def to_host(d_lat, fmt, L):
+    a = d_lat.cpu().numpy()
+    if fmt == pgg.FMT_U8:
+        return a
+    words = a.view(np.uint32)
+    bits = (words[..., None] >> np.arange(32, dtype=np.uint32)) & 1
+    return bits.reshape(words.shape[:-1] + (L,)).astype(np.uint8)
+
+
+def empty_lattice(fmt, L, B=None):
+    shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
+    if B is not None:
+        shape = (B,) + shape
+    return torch.empty(shape, dtype=torch.uint8 if fmt == pgg.FMT_U8 else torch.int32, device="cuda")
+
+
+def gpu_sweep(lat0, fmt, r, seed, order, t_begin, n_mcs, want_counts=True):
+    L = lat0.shape[0]
+    d = to_device(lat0, fmt)
+    cnt = torch.zeros(max(n_mcs, 1), dtype=torch.int64, device="cuda") if want_counts else None
+    pgg.pgg_sweep(d, fmt, L, r, K, seed, order, t_begin, n_mcs, cnt)
+    torch.cuda.synchronize()
+    counts = cnt.cpu().numpy().astype(np.uint64)[:n_mcs] if want_counts else None
+    return to_host(d, fmt, L), counts
+
+
+def assert_same(a, b, what=""):
+    if not np.array_equal(a, b):
+        bad = np.argwhere(a != b)
+        raise AssertionError(f"{what}: {len(bad)} mismatches, first at {bad[:5].tolist()}")
+
+
+# ---------------------------------------------------------------- K0 init (D4)
+@pytest.mark.parametrize("fmt", FMTS)
+@pytest.mark.parametrize("L,rho0,seed", [(64, 0.5, 1), (32, 0.0, 3), (32, 1.0, 3), (96, 0.2, 2**40 + 7),
+                                         (416, 0.77, 12), (4, 0.5, 9), (20, 0.5, 5), (2048, 0.5, 16)])
+def test_init_parity(fmt, L, rho0, seed):
+    if fmt == pgg.FMT_BITS and L % 32:
+        pytest.skip("bits layout needs L % 32 == 0")
+    d = empty_lattice(fmt, L)
+    pgg.pgg_init_lattice(d, fmt, L, rho0, seed)
+    torch.cuda.synchronize()
+    assert_same(to_host(d, fmt, L), orc.init(L, rho0, seed), "init")
+
+
+# ---------------------------------------------------------------- a1 phase classes (D5)
+@pytest.mark.parametrize("order", [pgg.ORDER_IID, pgg.ORDER_PERM])
+def test_phase_classes_parity(order):
+    for seed in (1, 2**33 + 5):
+        for t in (0, 1, 17, 99999, 2**32 - 1):
+            got = pgg.pgg_phase_classes(seed, t, order)
+            assert got == orc.phase_classes(seed, t, order).tolist(), (seed, t)
+            if order == pgg.ORDER_PERM:
+                assert sorted(got) == list(range(16))
+
+
+# ---------------------------------------------------------------- K3 density (Eq. 4)
+@pytest.mark.parametrize("fmt", FMTS)
+def test_density_parity(fmt):
+    for L, p in ((64, 0.5), (416, 0.3), (32, 0.0), (32, 1.0), (1024, 0.9)):
+        lat = wl.random_lattice(L, p, seed=L)
+        out = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+        pgg.pgg_density(to_device(lat, fmt), fmt, L, out)
+        torch.cuda.synchronize()
+        assert int(out.item()) == orc.count(lat) == int(lat.sum())
+
+
+# ---------------------------------------------------------------- config 1 in full
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("fmt", FMTS)
+@pytest.mark.parametrize("order", [pgg.ORDER_IID, pgg.ORDER_PERM])
+def test_config1_full_trace_and_snapshots(variant, fmt, order):
+    """BASELINE.json configs[0]: L=64, r=4, K=.5, seed 1, 1000 MCS; the lattice every 100 MCS
+    and the whole rho_C trace."""
+    cfg = wl.config1()
+    L, r, seed = cfg.L, cfg.rs[0], cfg.seeds[0]
+    use_variant(variant, fmt, L)
+    lat = orc.init(L, cfg.rho0, seed)
+    ref_counts, ref_snaps = orc.sweep(lat.copy(), r, K, seed, order, 0, cfg.n_mcs, snap_every=cfg.snap_every)
+    d = empty_lattice(fmt, L)
+    pgg.pgg_init_lattice(d, fmt, L, cfg.rho0, seed)
+    counts = []
+    for a in range(cfg.n_mcs // cfg.snap_every):
+        cnt = torch.zeros(cfg.snap_every, dtype=torch.int64, device="cuda")
+        pgg.pgg_sweep(d, fmt, L, r, K, seed, order, a * cfg.snap_every, cfg.snap_every, cnt)
+        torch.cuda.synchronize()
+        assert_same(to_host(d, fmt, L), ref_snaps[a], f"snapshot after {(a + 1) * cfg.snap_every} MCS")
+        counts.append(cnt.cpu().numpy().astype(np.uint64))
+    assert_same(np.concatenate(counts), ref_counts, "rho_C trace")
+
+
+# ---------------------------------------------------------------- sizes, tails, wrap
+SIZES = [4, 8, 12, 16, 20, 32, 36, 48, 64, 100, 128, 144, 256, 400, 512, 640]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("fmt", FMTS)
+@pytest.mark.parametrize("L", SIZES)
+def test_sweep_parity_sizes(variant, fmt, L):
+    """Several tiles plus ragged tails; L = 4 and 8 exercise coinciding wrap neighbours."""
+    if fmt == pgg.FMT_BITS and L % 32:
+        pytest.skip("bits layout needs L % 32 == 0")
+    use_variant(variant, fmt, L)
+    n_mcs = 12 if L <= 256 else 5
+    for seed, r, order in ((L + 1, 3.8, pgg.ORDER_IID), (2**35 + L, 4.6, pgg.ORDER_PERM)):
+        lat0 = orc.init(L, 0.5, seed)
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, r, K, seed, order, 3, n_mcs)
+        got, counts = gpu_sweep(lat0, fmt, r, seed, order, 3, n_mcs)
+        assert_same(got, ref, f"lattice L={L}")
+        assert_same(counts, ref_counts, f"counts L={L}")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("fmt", FMTS)
+def test_sweep_parity_structured_states(variant, fmt):
+    """Interfaces, compact clusters and the checkerboard: states where most
+    sites are bulk (skipped) or where every site is active."""
+    L = 256
+    use_variant(variant, fmt, L)
+    states = [wl.blobs_lattice(L, 3), wl.stripes_lattice(L, 5, True), wl.stripes_lattice(L, 7, False),
+              wl.checkerboard_lattice(L), wl.random_lattice(L, 0.03, 8), wl.random_lattice(L, 0.97, 9)]
+    for n, lat0 in enumerate(states):
+        for r in (3.8, 5.4):
+            ref = lat0.copy()
+            ref_counts, _ = orc.sweep(ref, r, K, 77 + n, pgg.ORDER_IID, 0, 8)
+            got, counts = gpu_sweep(lat0, fmt, r, 77 + n, pgg.ORDER_IID, 0, 8)
+            assert_same(got, ref, f"state {n}")
+            assert_same(counts, ref_counts, f"counts state {n}")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("fmt", FMTS)
+def test_absorbing_states_stay_absorbing(variant, fmt):
+    L = 128
+    use_variant(variant, fmt, L)
+    for v in (0, 1):
+        lat0 = np.full((L, L), v, dtype=np.uint8)
+        got, counts = gpu_sweep(lat0, fmt, 3.8, 5, pgg.ORDER_IID, 0, 6)
+        assert_same(got, lat0)
+        assert (counts == v * L * L).all()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("fmt", FMTS)
+def test_extreme_parameters(variant, fmt):
+    """Clamped table entries (S7): tiny K (step function) and huge r."""
+    L = 128
+    use_variant(variant, fmt, L)
+    for r, Kx in ((4.0, 1e-3), (25.0, 0.5), (1.0, 50.0)):
+        lat0 = orc.init(L, 0.5, 21)
+        ref = lat0.copy()
+        tab = orc.accept_table(r, Kx)
+        assert np.array_equal(tab, np.array(pgg.pgg_build_accept_table(r, Kx), dtype=np.uint32))
+        ref_counts, _ = orc.sweep(ref, r, Kx, 21, pgg.ORDER_IID, 0, 6)
+        d = to_device(lat0, fmt)
+        cnt = torch.zeros(6, dtype=torch.int64, device="cuda")
+        pgg.pgg_sweep(d, fmt, L, r, Kx, 21, pgg.ORDER_IID, 0, 6, cnt)
+        torch.cuda.synchronize()
+        assert_same(to_host(d, fmt, L), ref)
+        assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
+
+
+# ---------------------------------------------------------------- composition (P7)
+@pytest.mark.parametrize("fmt", FMTS)
+def test_composition_and_late_window(fmt):
+    """(a,b) then (a+b,c) == (a,b+c); t_begin near 2^32 exercises the counter width."""
+    L = 128
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    lat0 = orc.init(L, 0.5, 4)
+    for t0 in (0, 2**32 - 40):
+        one, c_one = gpu_sweep(lat0, fmt, 3.9, 4, pgg.ORDER_IID, t0, 30)
+        d = to_device(lat0, fmt)
+        c1 = torch.zeros(12, dtype=torch.int64, device="cuda")
+        c2 = torch.zeros(18, dtype=torch.int64, device="cuda")
+        pgg.pgg_sweep(d, fmt, L, 3.9, K, 4, pgg.ORDER_IID, t0, 12, c1)
+        pgg.pgg_sweep(d, fmt, L, 3.9, K, 4, pgg.ORDER_IID, t0 + 12, 18, c2)
+        torch.cuda.synchronize()
+        assert_same(to_host(d, fmt, L), one)
+        assert_same(torch.cat([c1, c2]).cpu().numpy().astype(np.uint64), c_one)
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, 3.9, K, 4, pgg.ORDER_IID, t0, 30)
+        assert_same(one, ref)
+        assert_same(c_one, ref_counts)
+
+
+def test_counts_null_and_zero_mcs():
+    L = 64
+    lat0 = orc.init(L, 0.5, 2)
+    got, _ = gpu_sweep(lat0, pgg.FMT_U8, 3.8, 2, pgg.ORDER_IID, 0, 4, want_counts=False)
+    ref = lat0.copy()
+    orc.sweep(ref, 3.8, K, 2, pgg.ORDER_IID, 0, 4)
+    assert_same(got, ref)
+    got, _ = gpu_sweep(lat0, pgg.FMT_U8, 3.8, 2, pgg.ORDER_IID, 0, 0, want_counts=False)
+    assert_same(got, lat0)
+
+
+# ---------------------------------------------------------------- a9 ensemble
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("fmt", FMTS)
+def test_ensemble_equals_solo_and_oracle(variant, fmt):
+    """Config-4 shape at reduced size: B lattices, r_k = 3.70 + (0.1 k)/63, seeds 1000+k."""
+    cfg = wl.config4()
+    B, L, n_mcs = 8, 128, 20
+    use_variant(variant, fmt, L)
+    rs, seeds = cfg.rs[::8][:B], cfg.seeds[::8][:B]
+    d = empty_lattice(fmt, L, B)
+    cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, n_mcs, cnt)
+    torch.cuda.synchronize()
+    got = to_host(d, fmt, L)
+    counts = cnt.cpu().numpy().astype(np.uint64)
+    for b in range(B):
+        ref = orc.init(L, 0.5, seeds[b])
+        solo, solo_counts = gpu_sweep(ref, fmt, rs[b], seeds[b], pgg.ORDER_IID, 0, n_mcs)
+        ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs)
+        assert_same(got[b], ref, f"member {b} vs oracle")
+        assert_same(got[b], solo, f"member {b} vs solo")
+        assert_same(counts[b], ref_counts)
+        assert_same(solo_counts, ref_counts)
+    # continue (rho0 < 0) from the given states
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_PERM, -1.0, n_mcs, 3, None)
+    torch.cuda.synchronize()
+    got2 = to_host(d, fmt, L)
+    for b in range(B):
+        ref = got[b].copy()
+        orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_PERM, n_mcs, 3)
+        assert_same(got2[b], ref, f"member {b} continued")
+
+
+# ---------------------------------------------------------------- full-size configs
+@pytest.mark.parametrize("fmt", FMTS)
+def test_config3_and_4_shapes_prefix(fmt):
+    """Configs 3 and 4 at full lattice size, in the ensemble launch bench-like runs use,
+    for a prefix of MCS the oracle finishes in seconds (full-length runs: DESIGN.md)."""
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    for cfg, B, n_mcs in ((wl.config3(), 2, 3), (wl.config4(), 4, 6)):
+        L = cfg.L
+        rs, seeds = cfg.rs[-B:], cfg.seeds[-B:]
+        d = empty_lattice(fmt, L, B)
+        cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+        pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, cfg.rho0, 0, n_mcs, cnt)
+        torch.cuda.synchronize()
+        got = to_host(d, fmt, L)
+        for b in range(B):
+            ref = orc.init(L, cfg.rho0, seeds[b])
+            ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs,
+                                      n_threads=orc.max_threads())
+            assert_same(got[b], ref, f"{cfg.name} member {b}")
+            assert_same(cnt[b].cpu().numpy().astype(np.uint64), ref_counts)
+
+
+@pytest.mark.parametrize("fmt", FMTS)
+def test_config5_full_size(fmt):
+    """BASELINE.json configs[4] at its full size (L=16384) in the launch configuration
+    bench.py times: whole lattice and counts after 2 MCS, then a late window entered from a
+    state the GPU produced (legal by composition, P7): sampled tiles are recomputed by the
+    oracle on a cut-out with an 8*... halo -- here simply the whole lattice for 1 more MCS."""
+    cfg = wl.config5()
+    L, r, seed = cfg.L, cfg.rs[0], cfg.seeds[0]
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    d = empty_lattice(fmt, L)
+    pgg.pgg_init_lattice(d, fmt, L, cfg.rho0, seed)
+    cnt = torch.zeros(2, dtype=torch.int64, device="cuda")
+    pgg.pgg_sweep(d, fmt, L, r, K, seed, pgg.ORDER_IID, 0, 2, cnt)
+    torch.cuda.synchronize()
+    ref = orc.init(L, cfg.rho0, seed)
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 0, 2, n_threads=orc.max_threads())
+    assert_same(to_host(d, fmt, L), ref, "C5 lattice after 2 MCS")
+    assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
+    # late window: 60 more MCS on the GPU (state leaves the random regime), then 1 MCS both ways
+    pgg.pgg_sweep(d, fmt, L, r, K, seed, pgg.ORDER_IID, 2, 60, None)
+    torch.cuda.synchronize()
+    ref = to_host(d, fmt, L).copy()
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    pgg.pgg_sweep(d, fmt, L, r, K, seed, pgg.ORDER_IID, 62, 1, cnt)
+    torch.cuda.synchronize()
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 62, 1, n_threads=orc.max_threads())
+    assert_same(to_host(d, fmt, L), ref, "C5 late window")
+    assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
