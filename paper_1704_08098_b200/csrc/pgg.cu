@@ -206,7 +206,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
                 if (variant == PGG_VARIANT_TILE) {
-                    pgg::tile_launch(plan, fmt, a, m, k, stream);
+                    pgg::tile_launch(plan, fmt, a, m, k, B, stream);
                 } else {
                     const uint32_t n_cls = (L / 4) * (L / 4);
                     dim3 grid((n_cls + 255) / 256, B);
