@@ -18,6 +18,8 @@
 // In-place writes are race-free (S1): nothing within Manhattan distance 3 of
 // an active site is written in the same phase.
 #pragma once
+#include <cstdlib>
+
 #include "pgg_common.cuh"
 
 namespace pgg {
@@ -369,9 +371,9 @@ inline int tile_plan(int fmt, uint32_t L, uint32_t B, TilePlan* p)
         if (e != cudaSuccess) return (int)e;
         e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_tile_kernel<kFmtU8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        e = cudaFuncSetAttribute(phase_tile_kernel<kFmtU8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 1024);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_tile_kernel<kFmtBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        e = cudaFuncSetAttribute(phase_tile_kernel<kFmtBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 1024);
         if (e != cudaSuccess) return (int)e;
         cudaFuncSetAttribute(phase_tile_kernel<kFmtU8>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         cudaFuncSetAttribute(phase_tile_kernel<kFmtBits>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
@@ -381,11 +383,17 @@ inline int tile_plan(int fmt, uint32_t L, uint32_t B, TilePlan* p)
     p->n_rowblocks = (L + kTileTH - 1) / kTileTH;
     p->n_tiles = p->n_strips * p->n_rowblocks;
     const uint32_t fixed = kTileWarps * kTileQueueCap * 4 + 160 * 4 + kTileMaxStages * 8 + 128;
-    // two CTAs per SM, each with as many stages as fit (>= 2)
+    // CTAs per SM and stages per CTA: as many stages as fit beside `cps` CTAs (>= 2).
+    // PGG_TILE_CTAS_PER_SM / PGG_TILE_STAGES override the defaults (tuning knobs).
+    uint32_t cps = 2, want_stages = 3;
+    if (const char* e = getenv("PGG_TILE_CTAS_PER_SM")) cps = (uint32_t)atoi(e);
+    if (const char* e = getenv("PGG_TILE_STAGES")) want_stages = (uint32_t)atoi(e);
+    if (cps < 1) cps = 1;
+    if (want_stages > (uint32_t)kTileMaxStages) want_stages = kTileMaxStages;
     uint32_t stages = 2;
-    const uint32_t per_cta = (uint32_t)(228 * 1024 / 2) - 2048;
-    while (stages < 3 && fixed + (stages + 1) * kTileStageBytes <= per_cta) ++stages;
-    uint32_t ctas = 2u * (uint32_t)sm_count;
+    const uint32_t per_cta = (uint32_t)(228 * 1024 / cps) - 1024 - 128;
+    while (stages < want_stages && fixed + (stages + 1) * kTileStageBytes <= per_cta) ++stages;
+    uint32_t ctas = cps * (uint32_t)sm_count;
     uint32_t gx = p->n_tiles < ctas ? p->n_tiles : ctas;
     if (B > 1) {  // share the machine between lattices
         uint32_t per_lat = (ctas + B - 1) / B;
