@@ -154,7 +154,7 @@ def run_ours(args):
     L, n_mcs = args.L, args.mcs
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
-               "fused": pgg.VARIANT_FUSED}[args.variant]
+               "fused": pgg.VARIANT_FUSED, "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND}[args.variant]
     pgg.pgg_set_variant(variant)
     seed = SEED + rank
     shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
@@ -303,7 +303,7 @@ def main():
     ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
-    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

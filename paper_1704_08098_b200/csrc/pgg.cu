@@ -16,6 +16,8 @@
 #include "pgg_common.cuh"
 #include "pgg_kernels_v0.cuh"
 #include "pgg_kernels_tile.cuh"
+#include "pgg_kernels_pipe.cuh"
+#include "pgg_kernels_band.cuh"
 
 namespace {
 
@@ -138,8 +140,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
 
     int variant = g_variant.load();
     const bool tile_ok = pgg::tile_supported(fmt, L);
-    if (variant == PGG_VARIANT_AUTO) variant = tile_ok ? PGG_VARIANT_TILE : PGG_VARIANT_V0;
-    if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_FUSED) && !tile_ok)
+    const bool band_ok = pgg::band_supported(fmt, L);
+    if (variant == PGG_VARIANT_AUTO) variant = band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
+    if (variant == PGG_VARIANT_BAND && !band_ok)
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
+    if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_FUSED || variant == PGG_VARIANT_PIPE) && !tile_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_FUSED) return fail(PGG_ERR_UNSUPPORTED, "fused variant not built");
     g_variant_used = variant;
@@ -193,6 +198,15 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     a.t_begin = t_begin;
 
     pgg::TilePlan plan;
+    pgg::BandPlan bplan;
+    if (variant == PGG_VARIANT_BAND) {
+        int32_t rc = pgg::band_plan(fmt, L, B, &bplan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "band kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
+    if (variant == PGG_VARIANT_PIPE) {
+        int32_t rc = pgg::pipe_plan(fmt, L, B, &plan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "pipe kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
     if (variant == PGG_VARIANT_TILE) {
         int32_t rc = pgg::tile_plan(fmt, L, B, &plan);
         if (rc != 0) return fail(PGG_ERR_CUDA, "tile kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
@@ -205,7 +219,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         PGG_LAUNCHED();
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
-                if (variant == PGG_VARIANT_TILE) {
+                if (variant == PGG_VARIANT_BAND) {
+                    pgg::band_launch(bplan, fmt, a, m, k, B, stream);
+                } else if (variant == PGG_VARIANT_PIPE) {
+                    pgg::pipe_launch(plan, fmt, a, m, k, B, stream);
+                } else if (variant == PGG_VARIANT_TILE) {
                     pgg::tile_launch(plan, fmt, a, m, k, B, stream);
                 } else {
                     const uint32_t n_cls = (L / 4) * (L / 4);
@@ -318,7 +336,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_FUSED)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_BAND)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -331,7 +349,8 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (fmt != PGG_FMT_U8 && fmt != PGG_FMT_BITS) return 0;
     if (L < 4 || L % 4 != 0 || L >= 65536 || (fmt == PGG_FMT_BITS && L % 32 != 0)) return 0;
     if (variant == PGG_VARIANT_AUTO || variant == PGG_VARIANT_V0) return 1;
-    if (variant == PGG_VARIANT_TILE) return pgg::tile_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_PIPE) return pgg::tile_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_BAND) return pgg::band_supported(fmt, L) ? 1 : 0;
     return 0;
 }
 
