@@ -125,16 +125,17 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
     const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
     const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
+    const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8u * NS, bar_mirror = bar_full + 16u * NS;
 
     for (int q = threadIdx.x; q < kTableSize; q += kBandThreads)
         tbl[q] = a.tables[(size_t)b * kTableSize + q];
     if (threadIdx.x == 0) {
         delta_cta = 0;
         for (uint32_t s = 0; s < NS; ++s) {
-            mbar_init(smem_u32(&bars[s]), 1);
-            mbar_init(smem_u32(&bars[NS + s]), kBandConsumers);
+            mbar_init(bar_full + 8u * s, 1);
+            mbar_init(bar_empty + 8u * s, kBandConsumers);
         }
-        mbar_init(smem_u32(&bars[2 * NS]), 1);
+        mbar_init(bar_mirror, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -153,18 +154,18 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
         const bool left_edge = j0b == 0, right_edge = j0b + wb == rb;
         const uint32_t ring_s = smem_u32(ring0);
         const uint32_t n_chunks = n_steps ? n_steps + 1 : 0;
+        // first lattice row of chunk kc: the first active row of step S0 + kc - 1 (mod L)
+        int row0 = (int)(((long long)RC * ((long long)S0 - 1) + ci) % (long long)L);
+        if (row0 < 0) row0 += (int)L;
+        uint32_t slot = 0, use = 0;  // chunk kc lives in slot kc % NS, use = kc / NS
         for (uint32_t kc = 0; kc < n_chunks; ++kc) {
-            const uint32_t slot = kc % NS;
-            if (kc >= NS) mbar_wait(smem_u32(&bars[NS + slot]), ((kc / NS) - 1u) & 1u);
-            const uint32_t bar = smem_u32(&bars[slot]);
+            if (use > 0) mbar_wait(bar_empty + 8u * slot, (use - 1u) & 1u);
+            const uint32_t bar = bar_full + 8u * slot;
             const int r_lo = kc == 0 ? RC - 3 : 0;  // of the prologue chunk only the tail is read
             if (lane == 0) mbar_expect_tx(bar, (uint32_t)((RC - r_lo) * (wb + 2 * kBandHaloB)));
             __syncwarp();
-            // first lattice row of chunk kc: the first active row of step S0 + kc - 1
-            const long long base = (long long)RC * ((long long)S0 + kc - 1) + ci;
             for (int rr = r_lo + lane; rr < RC; rr += 32) {
-                long long gi = (base + rr) % (long long)L;
-                if (gi < 0) gi += L;
+                const int gi = (int)((uint32_t)(row0 + rr) % L);
                 const uint8_t* src = lat + (size_t)gi * (size_t)rb;
                 const uint32_t dst = ring_s + (slot * (uint32_t)RC + (uint32_t)rr) * (uint32_t)pitch;
                 if (!left_edge && !right_edge) {
@@ -182,38 +183,76 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                 }
             }
             // chunk kc just went to slot 0: mirror the tail of slot NS-1 (chunk kc-1) in front of it
+            // (the mirror's previous readers released chunk kc-1-NS, which this warp waited for
+            // before it re-armed slot NS-1)
             if (kc >= 1 && slot == 0) {
-                mbar_wait(smem_u32(&bars[NS - 1]), ((kc - 1u) / NS) & 1u);
+                mbar_wait(bar_full + 8u * (NS - 1u), (use - 1u) & 1u);
                 const uint4* srcm = reinterpret_cast<const uint4*>(ring0 + (size_t)NS * g.slot_bytes - 3 * pitch);
                 uint4* dstm = reinterpret_cast<uint4*>(smem_raw);
-                for (int i = lane; i < 3 * pitch / 16; i += 32) dstm[i] = srcm[i];
+                const int n16 = 3 * pitch / 16;
+                int i = lane;
+                for (; i + 7 * 32 < n16; i += 8 * 32) {
+                    uint4 v[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) v[j] = srcm[i + 32 * j];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) dstm[i + 32 * j] = v[j];
+                }
+                for (; i < n16; i += 32) dstm[i] = srcm[i];
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&bars[2 * NS]));
+                if (lane == 0) mbar_arrive(bar_mirror);
             }
+            row0 += RC;
+            if (row0 >= (int)L) row0 %= (int)L;
+            if (++slot == NS) { slot = 0; ++use; }
         }
     } else {
         // ---------------- consumer warps ----------------
         const StepKey sk = make_step_key(a.seeds[b], a.t_begin + m, k, cls);
         uint32_t* q = queues + warp * kBandQueueCap;
-        constexpr uint32_t qmask = kBandQueueCap - 1;
         const uint32_t lt = (1u << lane) - 1u;
         const int rho = warp >> g.tpr_log2, tau = warp & ((1 << g.tpr_log2) - 1);
         const int colb = tau * kBandTaskB + 16 * lane;  // first core byte of this lane's 16
         const bool in = colb < wb;
         const int j0 = (FMT == kFmtU8) ? j0b : j0b * 8;
         const int rc_mask = RC - 1;
-        uint32_t head = 0, tail = 0, prev_tail = 0;
+        // the queue is linear: entries [0, qn); the first n_prev of them were queued by the previous step
+        uint32_t qn = 0, n_prev = 0;
         int delta = 0;
+        uint32_t slot = 1 % NS, use = 1 / NS;       // of chunk s + 1
+        uint32_t rel_slot = 0;                      // slot of chunk s - 1
+        uint32_t mir_par = 0;
+        int grow_cur = RC * (int)S0 + ci;           // lattice row of the step's first active row
+        uint32_t group = S0 * g.R + (uint32_t)rho;  // index of this warp's active row among the class rows
 
+        auto run_batches = [&](uint32_t par) {
+            // full batches from the front; the leftover (< 32) moves to the front
+            uint32_t head = 0;
+            while (qn - head >= 32u) {
+                delta += band_process<FMT>(q[head + lane], par, ring0, pitch, rc_mask, grow_cur, grow_cur - RC, j0,
+                                           lat, L, sk, tbl);
+                head += 32u;
+            }
+            if (head) {
+                const uint32_t left = qn - head;
+                uint32_t e = 0;
+                if ((uint32_t)lane < left) e = q[head + lane];
+                __syncwarp();
+                if ((uint32_t)lane < left) q[lane] = e;
+                __syncwarp();
+                qn = left;
+                n_prev = 0;
+            }
+        };
+
+        if (n_steps) mbar_wait(bar_full, 0u);
         for (uint32_t s = 0; s < n_steps; ++s) {
-            const uint32_t kc = s + 1, slot = kc % NS, par = s & 1u;
-            if (s == 0) mbar_wait(smem_u32(&bars[0]), 0u);
-            mbar_wait(smem_u32(&bars[slot]), (kc / NS) & 1u);
-            if (slot == 0) mbar_wait(smem_u32(&bars[2 * NS]), ((s / NS) & 1u));
-            const int grow_cur = RC * (int)(S0 + s) + ci;  // lattice row of the step's first active row
-            const int grow_prev = grow_cur - RC;
-            const uint32_t group = (S0 + s) * g.R + (uint32_t)rho;
-
+            const uint32_t par = s & 1u;
+            mbar_wait(bar_full + 8u * slot, use & 1u);
+            if (slot == 0) {
+                mbar_wait(bar_mirror, mir_par);
+                mir_par ^= 1u;
+            }
             if (group < g.n_groups) {
                 const int pos = (int)slot * RC + 4 * rho;  // ring row of this warp's active row
                 const uint8_t* rowp = ring0 + pos * pitch + kBandHaloB + colb;
@@ -230,6 +269,7 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                 const uint32_t u4[4] = {wu.x, wu.y, wu.z, wu.w};
                 const uint32_t d4[4] = {wd.x, wd.y, wd.z, wd.w};
                 const uint32_t ebase = (par << 31) | ((uint32_t)pos << 16);
+                uint32_t nb[4];
                 if (FMT == kFmtU8) {
                     // word w = sites 4w..4w+3 of this lane's 16; the active one is byte cj
                     const uint32_t bm = 0xFFu << (8 * cj);
@@ -237,17 +277,18 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                     for (int w = 0; w < 4; ++w) {
                         const uint32_t lw = __funnelshift_l(w == 0 ? pv : c4[w - 1], c4[w], 8);
                         const uint32_t rw = __funnelshift_r(c4[w], w == 3 ? nx : c4[w + 1], 8);
-                        const uint32_t nb = ((c4[w] ^ u4[w]) | (c4[w] ^ d4[w]) | (c4[w] ^ lw) | (c4[w] ^ rw)) & bm;  // S9
-                        const bool pred = nb != 0u;
-                        const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pred);
-                        if (pred) q[(tail + __popc(mk & lt)) & qmask] = ebase | (uint32_t)(colb + 4 * w + cj);
-                        tail += __popc(mk);
+                        nb[w] = ((c4[w] ^ u4[w]) | (c4[w] ^ d4[w]) | (c4[w] ^ lw) | (c4[w] ^ rw)) & bm;  // S9
                     }
-                    __syncwarp();
-                    while (tail - head >= 32u) {
-                        delta += band_process<FMT>(q[(head + lane) & qmask], par, ring0, pitch, rc_mask, grow_cur,
-                                                   grow_prev, j0, lat, L, sk, tbl);
-                        head += 32u;
+                    if (__any_sync(0xFFFFFFFFu, (nb[0] | nb[1] | nb[2] | nb[3]) != 0u)) {
+#pragma unroll
+                        for (int w = 0; w < 4; ++w) {
+                            const bool pred = nb[w] != 0u;
+                            const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pred);
+                            if (pred) q[qn + __popc(mk & lt)] = ebase | (uint32_t)(colb + 4 * w + cj);
+                            qn += __popc(mk);
+                        }
+                        __syncwarp();
+                        run_batches(par);
                     }
                 } else {
                     // word w = 32 sites; the 8 active ones are bits cj + 4 b
@@ -256,46 +297,47 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                     for (int w = 0; w < 4; ++w) {
                         const uint32_t lw = __funnelshift_l(w == 0 ? pv : c4[w - 1], c4[w], 1);
                         const uint32_t rw = __funnelshift_r(c4[w], w == 3 ? nx : c4[w + 1], 1);
-                        const uint32_t nb = ((c4[w] ^ u4[w]) | (c4[w] ^ d4[w]) | (c4[w] ^ lw) | (c4[w] ^ rw)) & cm;  // S9
-                        if (__any_sync(0xFFFFFFFFu, nb != 0u)) {
+                        nb[w] = ((c4[w] ^ u4[w]) | (c4[w] ^ d4[w]) | (c4[w] ^ lw) | (c4[w] ^ rw)) & cm;  // S9
+                    }
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) {
+                        if (__any_sync(0xFFFFFFFFu, nb[w] != 0u)) {
 #pragma unroll
                             for (int bb = 0; bb < 8; ++bb) {
                                 const int bit = cj + 4 * bb;
-                                const bool pred = (nb >> bit) & 1u;
+                                const bool pred = (nb[w] >> bit) & 1u;
                                 const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pred);
-                                if (pred)
-                                    q[(tail + __popc(mk & lt)) & qmask] = ebase | (uint32_t)(8 * (colb + 4 * w) + bit);
-                                tail += __popc(mk);
+                                if (pred) q[qn + __popc(mk & lt)] = ebase | (uint32_t)(8 * (colb + 4 * w) + bit);
+                                qn += __popc(mk);
                             }
                             __syncwarp();
-                            while (tail - head >= 32u) {
-                                delta += band_process<FMT>(q[(head + lane) & qmask], par, ring0, pitch, rc_mask,
-                                                           grow_cur, grow_prev, j0, lat, L, sk, tbl);
-                                head += 32u;
-                            }
+                            run_batches(par);
                         }
                     }
                 }
             }
             // sites of step s-1 still queued (then fewer than 32 are queued in all): flush them
-            if ((int32_t)(prev_tail - head) > 0) {
-                const uint32_t cnt = tail - head;
-                if ((uint32_t)lane < cnt)
-                    delta += band_process<FMT>(q[(head + lane) & qmask], par, ring0, pitch, rc_mask, grow_cur,
-                                               grow_prev, j0, lat, L, sk, tbl);
-                head = tail;
+            if (n_prev) {
+                if ((uint32_t)lane < qn)
+                    delta += band_process<FMT>(q[lane], par, ring0, pitch, rc_mask, grow_cur, grow_cur - RC, j0, lat, L,
+                                               sk, tbl);
+                qn = 0;
             }
             __syncwarp();
-            if (s > 0 && lane == 0) mbar_arrive(smem_u32(&bars[NS + (kc - 2u) % NS]));  // chunk s-1 is free
-            prev_tail = tail;
+            if (s > 0) {
+                if (lane == 0) mbar_arrive(bar_empty + 8u * rel_slot);  // chunk s-1 is free
+                if (++rel_slot == NS) rel_slot = 0;
+            }
+            n_prev = qn;
+            grow_cur += RC;
+            group += g.R;
+            if (++slot == NS) { slot = 0; ++use; }
         }
-        // drain: everything left belongs to the last step
-        if (n_steps) {
-            const uint32_t cnt = tail - head, s = n_steps - 1;
-            const int grow_cur = RC * (int)(S0 + s) + ci;
-            if ((uint32_t)lane < cnt)
-                delta += band_process<FMT>(q[(head + lane) & qmask], s & 1u, ring0, pitch, rc_mask, grow_cur,
-                                           grow_cur - RC, j0, lat, L, sk, tbl);
+        // drain: everything left was queued by the last step
+        if (qn) {
+            if ((uint32_t)lane < qn)
+                delta += band_process<FMT>(q[lane], (n_steps - 1u) & 1u, ring0, pitch, rc_mask, grow_cur - RC,
+                                           grow_cur - 2 * RC, j0, lat, L, sk, tbl);
         }
         if (a.deltas != nullptr) {
             delta = __reduce_add_sync(0xFFFFFFFFu, delta);
