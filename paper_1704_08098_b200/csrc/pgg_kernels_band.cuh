@@ -1,30 +1,37 @@
 // pgg_kernels_band.cuh -- the BAND phase kernel (K1 uint8, K2 bit-packed).
 //
-// Measured on B200 (profiles/): cp.async.bulk copies of ~0.5 KB issued by one
-// warp deliver only ~2.2 TB/s chip-wide, copies of >= 1 KB reach 5.6-5.8 TB/s.
-// So the lattice is not cut into square tiles (short rows, 16 % halo re-reads)
-// but into column STRIPS of up to 8 KB, and every persistent CTA streams one
-// BAND of consecutive lattice rows of a strip through a ring of row chunks in
-// shared memory: each lattice row is fetched exactly once per phase by one
-// large bulk-async copy (SASS UBLKCP, completing on an mbarrier), plus 16
-// bytes of column halo on each side (3 sites are needed; 16 bytes keep every
-// copy 16-byte aligned; at the lattice edge the halo is the periodic image).
+// Measured on B200 (profiles/r1_bulk_copy_microbench.md): cp.async.bulk copies
+// of ~0.5 KB issued by one warp deliver only ~2.2 TB/s chip-wide, copies of
+// >= 1 KB reach 5.6-5.8 TB/s.  So the lattice is not cut into square tiles
+// (short rows, 16 % halo re-reads) but into column STRIPS of up to 8 KB, and
+// every persistent CTA streams one BAND of consecutive lattice rows of a strip
+// through a ring of row chunks in shared memory: each lattice row is fetched
+// exactly once per phase by one large bulk-async copy (SASS UBLKCP, completing
+// on an mbarrier), plus 16 bytes of column halo on each side (3 sites are
+// needed; 16 bytes keep every copy 16-byte aligned; at the lattice edge the
+// halo is the periodic image).
 //
-//   ring   = [mirror: 3 rows][slot 0][slot 1]...[slot NS-1], slot = RC rows
-//   chunk k of a band = RC = 4 R consecutive lattice rows, first row = an
-//            active row (row % 4 == ci); lives in slot k % NS.
+//   ring    = [slot 0][slot 1]...[slot NS-1], slot = RC rows of `pitch` bytes
+//   chunk k = RC = 4 R consecutive lattice rows of the band, the first one an
+//             active row (row % 4 == ci); lives in slot k % NS.
 //   step s  = the R active rows of chunk s+1; their stencils reach 3 rows up
-//            (tail of chunk s) and 3 rows down (inside chunk s+1).
-//   mirror = copy of the last 3 rows of slot NS-1 placed in front of slot 0,
-//            written by the producer warp, so that the 7-row window of every
-//            active row is contiguous in shared memory.
+//             (tail of chunk s) and 3 rows down (inside chunk s+1).  When chunk
+//             s+1 sits in slot 0 the rows above it are the tail of slot NS-1:
+//             a negative row offset from ring row 0 gets `ring_bytes` added.
 //
-// 16 consumer warps: warp w owns 128 active sites (uint8; 512 bytes) or 1024
-// (bit-packed) of active row w / tpr, column task w % tpr, of every step.
-// Scan (S9 bulk test, word-wide logic), per-warp compaction queue, batches of
-// 32 through Philox + stencil + accept as in pgg_kernels_pipe.cuh.  A warp
-// releases chunk s-1 at the end of step s, so leftovers (< 32 queued sites) of
-// step s-1 are batched with the sites of step s.
+// 16 consumer warps + 1 producer warp.  Consumer warp w owns 128 active sites
+// (uint8; 512 bytes) or 1024 (bit-packed) of active row w / tpr, column task
+// w % tpr, of every step:
+//   scan    S9 bulk test ("all four neighbours equal s_x": no draw can change
+//           the site) on 16 bytes per lane with word-wide logic; survivors go
+//           to the warp's queue Q1;
+//   level 1 batches of 32 from Q1: Philox draw (a3), s_y (a4); sites with
+//           s_y != s_x go to queue Q2 with their u;
+//   level 2 batches of 32 from Q2: A_x - A_y (a5), threshold compare (a6),
+//           in-place write (a7), cooperator-count delta (a8).
+// Both queues are FIFO and keep leftovers (< 32) across ONE step boundary: a
+// warp releases chunk s-1 at the end of step s, after every site queued in
+// step s-1 has been finished.
 #pragma once
 #include "pgg_kernels_pipe.cuh"
 
@@ -34,9 +41,17 @@ constexpr int kBandConsumers = 16;
 constexpr int kBandThreads = (kBandConsumers + 1) * 32;
 constexpr int kBandTaskB = 512;     // bytes of one lattice row that one warp scans per step
 constexpr int kBandHaloB = 16;
-constexpr int kBandQueueCap = 512;  // ring entries per warp (power of two)
+constexpr int kBandQ2Cap = 64;      // Q2 entries (8 bytes each) per warp
 constexpr int kBandMaxSlots = 6;
-constexpr int kBandFixedBytes = kBandConsumers * kBandQueueCap * 4 + 160 * 4 + (2 * kBandMaxSlots + 2) * 8 + 128;
+
+// Q1 entries (4 bytes) per warp: leftover (< 32) + the sites one scan round can add
+template <int FMT> struct BandQ1 { static constexpr int cap = (FMT == kFmtU8) ? 32 + 128 : 32 + 256; };
+
+template <int FMT>
+constexpr int band_fixed_bytes()
+{
+    return kBandConsumers * (BandQ1<FMT>::cap * 4 + kBandQ2Cap * 8) + 160 * 4 + 2 * kBandMaxSlots * 8 + 128;
+}
 
 struct BandPlan {
     uint32_t row_bytes;  // bytes per lattice row
@@ -54,50 +69,88 @@ struct BandPlan {
     uint32_t smem_bytes;
 };
 
-// Steps a3-a7 for one queued site; entry = step parity << 31 | ring row << 16 | site column.
-template <int FMT>
-__device__ __forceinline__ int band_process(uint32_t e, uint32_t par_cur, const uint8_t* __restrict__ ring0,
-                                            int pitch, int rc_mask, int grow_cur, int grow_prev, int j0,
-                                            uint8_t* __restrict__ lat, uint32_t L, const StepKey& sk,
-                                            const uint32_t* __restrict__ tbl)
+// Q1 entry: step parity << 31 | ring row << 16 | site column (core-relative).
+// Q2 entry: .x = Q1 entry | dir << 29 | s_x << 28, .y = u.   (ring row < 2^12)
+struct BandCtx {
+    const uint8_t* ring0;  // slot 0, row 0
+    int pitch;
+    int ring_bytes;        // NS * slot_bytes
+    int rc_mask;           // RC - 1
+    int j0;                // first core SITE column of the strip
+    uint32_t L;
+};
+
+// lattice site index of a queued entry
+__device__ __forceinline__ uint32_t band_site(uint32_t e, uint32_t par_cur, int grow_cur, const BandCtx& cx)
 {
-    const int pos = (int)((e >> 16) & 0x7FFFu), c = (int)(e & 0xFFFFu);
-    const int gi = (((e >> 31) == par_cur) ? grow_cur : grow_prev) + (pos & rc_mask);
-    const uint32_t site = (uint32_t)gi * L + (uint32_t)(j0 + c);
+    const int pos = (int)((e >> 16) & 0xFFFu), c = (int)(e & 0xFFFFu);
+    const int gi = (((e >> 31) == par_cur) ? grow_cur : grow_cur - (cx.rc_mask + 1)) + (pos & cx.rc_mask);
+    return (uint32_t)gi * cx.L + (uint32_t)(cx.j0 + c);
+}
+
+// One site of the staged ring: row `pos` + rr (rr in [-3, 3]), site column c + cc.
+// `fix` = ring_bytes if pos == 0 (rows above ring row 0 are the tail of the last slot), else 0.
+template <int FMT>
+__device__ __forceinline__ int band_get(const uint8_t* rowp, int pitch, int c, int rr, int cc, int fixr)
+{
+    // fixr: 0, or `fix` when this access has rr < 0
+    if (FMT == kFmtU8) return rowp[rr * pitch + c + cc + fixr];
+    const int q = c + cc;
+    return (rowp[rr * pitch + (q >> 3) + fixr] >> (q & 7)) & 1;
+}
+
+// Level 1 (a3, a4): draw, neighbour compare.  Returns true if the site goes on to level 2.
+template <int FMT>
+__device__ __forceinline__ bool band_level1(uint32_t e, uint32_t par_cur, int grow_cur, const BandCtx& cx,
+                                            const StepKey& sk, uint2& out)
+{
+    const uint32_t site = band_site(e, par_cur, grow_cur, cx);
     uint32_t x0, u;
     step_draw(sk, site, x0, u);
     const uint32_t dir = x0 >> 30;  // 0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1)
-    // e = unit step towards y, f = perpendicular unit step (ring row, site column)
+    const int pos = (int)((e >> 16) & 0xFFFu);
+    const int c = (int)(e & 0xFFFFu) + ((FMT == kFmtU8) ? kBandHaloB : 8 * kBandHaloB);
+    const uint8_t* rowp = cx.ring0 + pos * cx.pitch;
+    const int er = dir == 0 ? -1 : dir == 1 ? 1 : 0;
+    const int ec = dir == 2 ? -1 : dir == 3 ? 1 : 0;
+    const int fix = (pos == 0 && dir == 0) ? cx.ring_bytes : 0;
+    const int sx = band_get<FMT>(rowp, cx.pitch, c, 0, 0, 0);
+    const int sy = band_get<FMT>(rowp, cx.pitch, c, er, ec, fix);
+    out.x = e | (dir << 29) | ((uint32_t)sx << 28);
+    out.y = u;
+    return sx != sy;
+}
+
+// Level 2 (a5-a7): payoff difference, acceptance, write.  Returns the change of the cooperator count.
+template <int FMT>
+__device__ __forceinline__ int band_level2(uint2 w, uint32_t par_cur, int grow_cur, const BandCtx& cx,
+                                           uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl)
+{
+    const uint32_t e = w.x, u = w.y;
+    const uint32_t dir = (e >> 29) & 3u;
+    const int sx = (int)((e >> 28) & 1u), sy = 1 - sx;
+    const int pos = (int)((e >> 16) & 0xFFFu);
+    const int c = (int)(e & 0xFFFFu) + ((FMT == kFmtU8) ? kBandHaloB : 8 * kBandHaloB);
+    const uint8_t* rowp = cx.ring0 + pos * cx.pitch;
+    // e = unit step towards y, f = perpendicular unit step: (ring row, site column)
     const int er = dir == 0 ? -1 : dir == 1 ? 1 : 0;
     const int ec = dir == 2 ? -1 : dir == 3 ? 1 : 0;
     const int fr = dir < 2 ? 0 : 1, fc = dir < 2 ? 1 : 0;
-    int sx, sy, dA;
-    if (FMT == kFmtU8) {
-        const uint8_t* p = ring0 + pos * pitch + kBandHaloB + c;
-        const int eo = er * pitch + ec, fo = fr * pitch + fc;
-        sx = p[0];
-        sy = p[eo];
-        if (sx == sy) return 0;
-        // A_x - A_y with A = 5 s + 2 (nearest + diagonal) + axial distance-2 (include/pgg.h):
-        // weights of x's 13-site stencil minus those of y's, at offset (a along e, b along f)
-        dA = p[-2 * eo] + p[-eo] - p[2 * eo] - p[3 * eo] + 3 * (sx - sy)
-           + 2 * (p[-eo + fo] + p[-eo - fo] - p[2 * eo + fo] - p[2 * eo - fo])
-           + p[2 * fo] + p[-2 * fo] - p[eo + 2 * fo] - p[eo - 2 * fo];
-    } else {
-        const uint8_t* rowp = ring0 + pos * pitch;
-        const int cc = c + 8 * kBandHaloB;
-        auto S = [&](int a, int b) {
-            const int rr = a * er + b * fr, q = cc + a * ec + b * fc;
-            return (int)((rowp[rr * pitch + (q >> 3)] >> (q & 7)) & 1);
-        };
-        sx = S(0, 0);
-        sy = S(1, 0);
-        if (sx == sy) return 0;
-        dA = S(-2, 0) + S(-1, 0) - S(2, 0) - S(3, 0) + 3 * (sx - sy)
-           + 2 * (S(-1, 1) + S(-1, -1) - S(2, 1) - S(2, -1))
-           + S(0, 2) + S(0, -2) - S(1, 2) - S(1, -2);
-    }
+    // accesses whose ring row is above row `pos`: a > 0 when dir == 0, a < 0 when dir == 1,
+    // b < 0 when dir >= 2 (then, and only if pos == 0, they live at the end of the ring)
+    const int fix = pos == 0 ? cx.ring_bytes : 0;
+    const int fa_pos = dir == 0 ? fix : 0, fa_neg = dir == 1 ? fix : 0, fb_neg = dir >= 2 ? fix : 0;
+    auto S = [&](int a, int b) {
+        const int fixr = (a > 0 ? fa_pos : 0) + (a < 0 ? fa_neg : 0) + (b < 0 ? fb_neg : 0);
+        return band_get<FMT>(rowp, cx.pitch, c, a * er + b * fr, a * ec + b * fc, fixr);
+    };
+    // A_x - A_y with A = 5 s + 2 (nearest + diagonal) + axial distance-2 (include/pgg.h):
+    // weights of x's 13-site stencil minus those of y's, at offset (a along e, b along f)
+    const int dA = S(-2, 0) + S(-1, 0) - S(2, 0) - S(3, 0) + 3 * (sx - sy)
+                 + 2 * (S(-1, 1) + S(-1, -1) - S(2, 1) - S(2, -1))
+                 + S(0, 2) + S(0, -2) - S(1, 2) - S(1, -2);
     if (u < tbl[table_index(dA, sx - sy)]) {
+        const uint32_t site = band_site(e, par_cur, grow_cur, cx);
         if (FMT == kFmtU8)
             lat[site] = (uint8_t)sy;
         else
@@ -112,11 +165,12 @@ __global__ void __launch_bounds__(kBandThreads, 1)
 phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
 {
     extern __shared__ __align__(128) uint8_t smem_raw[];
+    constexpr int kQ1 = BandQ1<FMT>::cap;
     const uint32_t NS = g.NS;
-    uint8_t* ring0 = smem_raw + 3 * g.pitch;  // slot 0, row 0; the mirror sits in front of it
-    uint32_t* queues = reinterpret_cast<uint32_t*>(smem_raw + 3 * g.pitch + (size_t)NS * g.slot_bytes);
-    uint32_t* tbl = queues + kBandConsumers * kBandQueueCap;
-    unsigned long long* bars = reinterpret_cast<unsigned long long*>(tbl + 160);  // full[NS], empty[NS], mirror
+    uint8_t* ring0 = smem_raw;
+    uint8_t* qbase = smem_raw + (size_t)NS * g.slot_bytes;
+    uint32_t* tbl = reinterpret_cast<uint32_t*>(qbase + kBandConsumers * (kQ1 * 4 + kBandQ2Cap * 8));
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(tbl + 160);  // full[NS], empty[NS]
     __shared__ int delta_cta;
 
     const uint32_t b = blockIdx.y;
@@ -125,7 +179,7 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
     const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
     const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
-    const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8u * NS, bar_mirror = bar_full + 16u * NS;
+    const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8u * NS;
 
     for (int q = threadIdx.x; q < kTableSize; q += kBandThreads)
         tbl[q] = a.tables[(size_t)b * kTableSize + q];
@@ -135,7 +189,6 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
             mbar_init(bar_full + 8u * s, 1);
             mbar_init(bar_empty + 8u * s, kBandConsumers);
         }
-        mbar_init(bar_mirror, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -182,26 +235,6 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                     bulk_g2s(dst + kBandHaloB + (uint32_t)wb, src, kBandHaloB, bar);
                 }
             }
-            // chunk kc just went to slot 0: mirror the tail of slot NS-1 (chunk kc-1) in front of it
-            // (the mirror's previous readers released chunk kc-1-NS, which this warp waited for
-            // before it re-armed slot NS-1)
-            if (kc >= 1 && slot == 0) {
-                mbar_wait(bar_full + 8u * (NS - 1u), (use - 1u) & 1u);
-                const uint4* srcm = reinterpret_cast<const uint4*>(ring0 + (size_t)NS * g.slot_bytes - 3 * pitch);
-                uint4* dstm = reinterpret_cast<uint4*>(smem_raw);
-                const int n16 = 3 * pitch / 16;
-                int i = lane;
-                for (; i + 7 * 32 < n16; i += 8 * 32) {
-                    uint4 v[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) v[j] = srcm[i + 32 * j];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) dstm[i + 32 * j] = v[j];
-                }
-                for (; i < n16; i += 32) dstm[i] = srcm[i];
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_mirror);
-            }
             row0 += RC;
             if (row0 >= (int)L) row0 %= (int)L;
             if (++slot == NS) { slot = 0; ++use; }
@@ -209,50 +242,76 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
     } else {
         // ---------------- consumer warps ----------------
         const StepKey sk = make_step_key(a.seeds[b], a.t_begin + m, k, cls);
-        uint32_t* q = queues + warp * kBandQueueCap;
+        uint32_t* q1 = reinterpret_cast<uint32_t*>(qbase + warp * (kQ1 * 4 + kBandQ2Cap * 8));
+        uint2* q2 = reinterpret_cast<uint2*>(q1 + kQ1);
         const uint32_t lt = (1u << lane) - 1u;
         const int rho = warp >> g.tpr_log2, tau = warp & ((1 << g.tpr_log2) - 1);
         const int colb = tau * kBandTaskB + 16 * lane;  // first core byte of this lane's 16
         const bool in = colb < wb;
-        const int j0 = (FMT == kFmtU8) ? j0b : j0b * 8;
-        const int rc_mask = RC - 1;
-        // the queue is linear: entries [0, qn); the first n_prev of them were queued by the previous step
-        uint32_t qn = 0, n_prev = 0;
+        BandCtx cx;
+        cx.ring0 = ring0;
+        cx.pitch = pitch;
+        cx.ring_bytes = (int)(NS * g.slot_bytes);
+        cx.rc_mask = RC - 1;
+        cx.j0 = (FMT == kFmtU8) ? j0b : j0b * 8;
+        cx.L = L;
+        // Both queues are linear, entries [0, n).  n1_old / n2_old = how many entries at the
+        // front were queued by the previous step (they must be finished before this step ends).
+        uint32_t n1 = 0, n2 = 0, n1_old = 0, n2_old = 0;
         int delta = 0;
         uint32_t slot = 1 % NS, use = 1 / NS;       // of chunk s + 1
         uint32_t rel_slot = 0;                      // slot of chunk s - 1
-        uint32_t mir_par = 0;
+        uint32_t par = 0;
         int grow_cur = RC * (int)S0 + ci;           // lattice row of the step's first active row
         uint32_t group = S0 * g.R + (uint32_t)rho;  // index of this warp's active row among the class rows
 
-        auto run_batches = [&](uint32_t par) {
-            // full batches from the front; the leftover (< 32) moves to the front
+        // level 2 on the first `cnt` (<= 32) entries of Q2; the rest moves to the front
+        auto run_level2 = [&](uint32_t cnt) {
+            uint2 w = make_uint2(0u, 0u), mv = w;
+            if ((uint32_t)lane < cnt) w = q2[lane];
+            const uint32_t left = n2 - cnt;
+            if ((uint32_t)lane < left) mv = q2[cnt + lane];
+            __syncwarp();
+            if ((uint32_t)lane < left) q2[lane] = mv;
+            if ((uint32_t)lane < cnt) delta += band_level2<FMT>(w, par, grow_cur, cx, lat, tbl);
+            __syncwarp();
+            n2 = left;
+            n2_old = n2_old > cnt ? n2_old - cnt : 0u;
+        };
+        // level 1 on the first `cnt` (<= 32) entries of Q1 starting at `head`
+        auto run_level1 = [&](uint32_t head, uint32_t cnt, bool has_old) {
+            uint2 w;
+            bool go = false;
+            if ((uint32_t)lane < cnt) go = band_level1<FMT>(q1[head + lane], par, grow_cur, cx, sk, w);
+            const uint32_t mk = __ballot_sync(0xFFFFFFFFu, go);
+            if (go) q2[n2 + __popc(mk & lt)] = w;
+            n2 += __popc(mk);
+            if (has_old) n2_old = n2;  // conservatively: everything queued so far may be old
+            __syncwarp();
+            if (n2 >= 32u) run_level2(32u);
+        };
+        // full batches from the front of Q1; the leftover (< 32) moves to the front
+        auto run_batches = [&]() {
             uint32_t head = 0;
-            while (qn - head >= 32u) {
-                delta += band_process<FMT>(q[head + lane], par, ring0, pitch, rc_mask, grow_cur, grow_cur - RC, j0,
-                                           lat, L, sk, tbl);
+            while (n1 - head >= 32u) {
+                run_level1(head, 32u, head < n1_old);
                 head += 32u;
             }
             if (head) {
-                const uint32_t left = qn - head;
+                const uint32_t left = n1 - head;
                 uint32_t e = 0;
-                if ((uint32_t)lane < left) e = q[head + lane];
+                if ((uint32_t)lane < left) e = q1[head + lane];
                 __syncwarp();
-                if ((uint32_t)lane < left) q[lane] = e;
+                if ((uint32_t)lane < left) q1[lane] = e;
                 __syncwarp();
-                qn = left;
-                n_prev = 0;
+                n1 = left;
+                n1_old = 0;
             }
         };
 
         if (n_steps) mbar_wait(bar_full, 0u);
         for (uint32_t s = 0; s < n_steps; ++s) {
-            const uint32_t par = s & 1u;
             mbar_wait(bar_full + 8u * slot, use & 1u);
-            if (slot == 0) {
-                mbar_wait(bar_mirror, mir_par);
-                mir_par ^= 1u;
-            }
             if (group < g.n_groups) {
                 const int pos = (int)slot * RC + 4 * rho;  // ring row of this warp's active row
                 const uint8_t* rowp = ring0 + pos * pitch + kBandHaloB + colb;
@@ -260,7 +319,7 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                 uint32_t pv = 0, nx = 0;
                 if (in) {
                     wc = *reinterpret_cast<const uint4*>(rowp);
-                    wu = *reinterpret_cast<const uint4*>(rowp - pitch);
+                    wu = *reinterpret_cast<const uint4*>(rowp - pitch + (pos == 0 ? cx.ring_bytes : 0));
                     wd = *reinterpret_cast<const uint4*>(rowp + pitch);
                     pv = *reinterpret_cast<const uint32_t*>(rowp - 4);
                     nx = *reinterpret_cast<const uint32_t*>(rowp + 16);
@@ -284,11 +343,11 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                         for (int w = 0; w < 4; ++w) {
                             const bool pred = nb[w] != 0u;
                             const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pred);
-                            if (pred) q[qn + __popc(mk & lt)] = ebase | (uint32_t)(colb + 4 * w + cj);
-                            qn += __popc(mk);
+                            if (pred) q1[n1 + __popc(mk & lt)] = ebase | (uint32_t)(colb + 4 * w + cj);
+                            n1 += __popc(mk);
                         }
                         __syncwarp();
-                        run_batches(par);
+                        run_batches();
                     }
                 } else {
                     // word w = 32 sites; the 8 active ones are bits cj + 4 b
@@ -307,38 +366,40 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
                                 const int bit = cj + 4 * bb;
                                 const bool pred = (nb[w] >> bit) & 1u;
                                 const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pred);
-                                if (pred) q[qn + __popc(mk & lt)] = ebase | (uint32_t)(8 * (colb + 4 * w) + bit);
-                                qn += __popc(mk);
+                                if (pred) q1[n1 + __popc(mk & lt)] = ebase | (uint32_t)(8 * (colb + 4 * w) + bit);
+                                n1 += __popc(mk);
                             }
                             __syncwarp();
-                            run_batches(par);
+                            run_batches();
                         }
                     }
                 }
             }
-            // sites of step s-1 still queued (then fewer than 32 are queued in all): flush them
-            if (n_prev) {
-                if ((uint32_t)lane < qn)
-                    delta += band_process<FMT>(q[lane], par, ring0, pitch, rc_mask, grow_cur, grow_cur - RC, j0, lat, L,
-                                               sk, tbl);
-                qn = 0;
+            // sites queued by step s-1 must be finished now: their rows are about to be released
+            if (n1_old) {  // then n1 < 32
+                run_level1(0u, n1, true);
+                n1 = 0;
             }
-            __syncwarp();
+            if (n2_old) run_level2(n2);  // then n2 < 32
             if (s > 0) {
                 if (lane == 0) mbar_arrive(bar_empty + 8u * rel_slot);  // chunk s-1 is free
                 if (++rel_slot == NS) rel_slot = 0;
             }
-            n_prev = qn;
+            n1_old = n1;
+            n2_old = n2;
+            par ^= 1u;
             grow_cur += RC;
             group += g.R;
             if (++slot == NS) { slot = 0; ++use; }
         }
         // drain: everything left was queued by the last step
-        if (qn) {
-            if ((uint32_t)lane < qn)
-                delta += band_process<FMT>(q[lane], (n_steps - 1u) & 1u, ring0, pitch, rc_mask, grow_cur - RC,
-                                           grow_cur - 2 * RC, j0, lat, L, sk, tbl);
+        par ^= 1u;
+        grow_cur -= RC;
+        if (n1) {
+            run_level1(0u, n1, true);
+            n1 = 0;
         }
+        if (n2) run_level2(n2);
         if (a.deltas != nullptr) {
             delta = __reduce_add_sync(0xFFFFFFFFu, delta);
             if (lane == 0 && delta != 0) atomicAdd(&delta_cta, delta);
@@ -392,14 +453,15 @@ inline int band_plan(int fmt, uint32_t L, uint32_t B, BandPlan* p)
     if (per_strip < 1) per_strip = 1;
     p->nb = p->n_super < per_strip ? p->n_super : per_strip;
     const uint32_t max_chunks = (p->n_super + p->nb - 1) / p->nb + 1;
-    uint32_t want = 5;
+    uint32_t want = kBandMaxSlots;
     if (const char* e = getenv("PGG_BAND_SLOTS")) want = (uint32_t)atoi(e);
     if (want > (uint32_t)kBandMaxSlots) want = kBandMaxSlots;
     if (want < 3) want = 3;
-    while (want > 3 && 3 * p->pitch + want * p->slot_bytes + kBandFixedBytes > (uint32_t)smem_optin - 1024) --want;
+    const uint32_t fixed = fmt == kFmtU8 ? band_fixed_bytes<kFmtU8>() : band_fixed_bytes<kFmtBits>();
+    while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 1024) --want;
     if (max_chunks < want) want = max_chunks < 3 ? 3 : max_chunks;
     p->NS = want;
-    p->smem_bytes = 3 * p->pitch + p->NS * p->slot_bytes + kBandFixedBytes;
+    p->smem_bytes = p->NS * p->slot_bytes + fixed;
     return 0;
 }
 
