@@ -302,9 +302,9 @@ def test_config3_and_4_shapes_prefix(fmt):
 @pytest.mark.parametrize("fmt", FMTS)
 def test_config5_full_size(fmt):
     """BASELINE.json configs[4] at its full size (L=16384) in the launch configuration
-    bench.py times: whole lattice and counts after 2 MCS, then a late window entered from a
-    state the GPU produced (legal by composition, P7): sampled tiles are recomputed by the
-    oracle on a cut-out with an 8*... halo -- here simply the whole lattice for 1 more MCS."""
+    bench.py times: whole lattice and counts after 2 MCS against a live oracle run.  Later
+    times (lattice hashes and the whole count trace of a stored oracle run) are checked in
+    tests/test_gpu_goldens.py; no GPU-produced state is ever handed to the oracle."""
     cfg = wl.config5()
     L, r, seed = cfg.L, cfg.rs[0], cfg.seeds[0]
     pgg.pgg_set_variant(pgg.VARIANT_AUTO)
@@ -316,14 +316,4 @@ def test_config5_full_size(fmt):
     ref = orc.init(L, cfg.rho0, seed)
     ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 0, 2, n_threads=orc.max_threads())
     assert_same(to_host(d, fmt, L), ref, "C5 lattice after 2 MCS")
-    assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
-    # late window: 60 more MCS on the GPU (state leaves the random regime), then 1 MCS both ways
-    pgg.pgg_sweep(d, fmt, L, r, K, seed, pgg.ORDER_IID, 2, 60, None)
-    torch.cuda.synchronize()
-    ref = to_host(d, fmt, L).copy()
-    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
-    pgg.pgg_sweep(d, fmt, L, r, K, seed, pgg.ORDER_IID, 62, 1, cnt)
-    torch.cuda.synchronize()
-    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 62, 1, n_threads=orc.max_threads())
-    assert_same(to_host(d, fmt, L), ref, "C5 late window")
     assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
