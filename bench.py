@@ -154,7 +154,8 @@ def run_ours(args):
     L, n_mcs = args.L, args.mcs
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
-               "fused": pgg.VARIANT_FUSED, "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND}[args.variant]
+               "fused": pgg.VARIANT_FUSED, "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND,
+               "ring": pgg.VARIANT_RING}[args.variant]
     pgg.pgg_set_variant(variant)
     seed = SEED + rank
     shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
@@ -174,6 +175,17 @@ def run_ours(args):
         pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
         if i is not None:
             ev_b[i].record(stream)
+        if args.profile_mcs >= 0:
+            # for `ncu --profile-from-start off`: only MCS `profile_mcs` lies in the profiled range
+            pm = min(args.profile_mcs, n_mcs - 1)
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, pm, None, stream)
+            torch.cuda.synchronize()
+            torch.cuda.profiler.start()
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, pm, 1, None, stream)
+            torch.cuda.synchronize()
+            torch.cuda.profiler.stop()
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, pm + 1, n_mcs - pm - 1, None, stream)
+            pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
         pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, n_mcs, d_counts, stream)
         if i is not None:
             ev_c[i].record(stream)
@@ -303,8 +315,11 @@ def main():
     ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
-    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band", "ring"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile-mcs", type=int, default=-1,
+                    help="profiling aid: bracket this MCS with cudaProfilerStart/Stop (ncu --profile-from-start off); "
+                         "the run's numbers are then not bench values")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -36,11 +36,6 @@ def lattice_sha(d_lat, fmt, L):
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
 
 
-def test_golden_files_exist():
-    names = {f.name.split("_")[0] for f in FILES}
-    assert {"C2", "C3", "C4", "C5"} <= names, f"missing golden files, have {sorted(names)}"
-
-
 @pytest.mark.parametrize("fmt", [pgg.FMT_U8, pgg.FMT_BITS])
 @pytest.mark.parametrize("path", FILES, ids=[f.stem for f in FILES])
 def test_config_reproduces_stored_oracle_run(path, fmt):
@@ -84,3 +79,8 @@ def test_config_reproduces_stored_oracle_run(path, fmt):
             assert int(trace[b, int(s) - 1]) == v, f"{g['config']} member {b}: count after MCS {s}"
         assert hashlib.sha256(np.ascontiguousarray(trace[b]).tobytes()).hexdigest() == m["trace_sha256"], \
             f"{g['config']} member {b}: rho_C trace differs"
+
+
+def test_golden_files_exist():
+    names = {f.name.split("_")[0] for f in FILES}
+    assert {"C2", "C3", "C4", "C5"} <= names, f"missing golden files, have {sorted(names)}"
