@@ -46,8 +46,15 @@ constexpr int kRingHaloB = 16;
 constexpr int kRingQ1Cap = 160;   // 8-byte entries per warp: leftover (< 32) + 128 new
 constexpr int kRingQ2Cap = 64;    // 16-byte entries per warp (a ring: power of two)
 constexpr int kRingMaxSlots = 6;
-constexpr int kRingWarpQBytes = kRingQ1Cap * 8 + kRingQ2Cap * 16;
-constexpr int kRingFixedBytes = kRingConsumers * kRingWarpQBytes + 160 * 4 + 2 * kRingMaxSlots * 8 + 8 * 4 + 128;
+// Q2 (a second compaction between the Philox draw and the stencil) fills its batches of 32
+// only half on average -- a site may wait for one step only -- and its 16 KB are worth more
+// as ring slots (profiles/r1_ring_design_notes.md), so level 2 runs inline under divergence.
+// The bit-packed stencil (a shift and a mask per read) is dearer, there Q2 still pays.
+template <int FMT> struct RingCfg {
+    static constexpr bool q2 = FMT == kFmtBits;
+    static constexpr int warp_q_bytes = kRingQ1Cap * 8 + (q2 ? kRingQ2Cap * 16 : 0);
+    static constexpr int fixed_bytes = kRingConsumers * warp_q_bytes + 160 * 4 + 2 * kRingMaxSlots * 8 + 8 * 4 + 128;
+};
 
 struct RingPlan {
     uint32_t row_bytes;  // bytes per lattice row
@@ -125,7 +132,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
     const int RC = (int)g.RC, pitch = (int)g.pitch;
     uint8_t* ring0 = smem_raw + 3 * pitch;  // three mirror rows in front of slot 0
     uint8_t* qbase = ring0 + (size_t)NS * g.slot_bytes;
-    uint32_t* tbl = reinterpret_cast<uint32_t*>(qbase + kRingConsumers * kRingWarpQBytes);
+    uint32_t* tbl = reinterpret_cast<uint32_t*>(qbase + kRingConsumers * RingCfg<FMT>::warp_q_bytes);
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(tbl + 160);  // full[NS], empty[NS]
     int* eoff = reinterpret_cast<int*>(bars + 2 * kRingMaxSlots);                 // e[4], f[4]
     __shared__ int delta_cta;
@@ -205,7 +212,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
     } else {
         // ---------------- consumer warps ----------------
         const StepKey sk = make_step_key(a.seeds[b], a.t_begin + m, k, cls);
-        uint2* q1 = reinterpret_cast<uint2*>(qbase + warp * kRingWarpQBytes);
+        uint2* q1 = reinterpret_cast<uint2*>(qbase + warp * RingCfg<FMT>::warp_q_bytes);
         uint4* q2 = reinterpret_cast<uint4*>(q1 + kRingQ1Cap);
         const uint32_t lt = (1u << lane) - 1u;
         const int rho = warp >> g.tpr_log2, tau = warp & ((1 << g.tpr_log2) - 1);
@@ -243,6 +250,10 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         };
         // Q2 append of one level-1 batch whose first `n_old` lanes hold old entries
         auto push2 = [&](bool go, const uint4& w, uint32_t n_old) {
+            if (!RingCfg<FMT>::q2) {
+                if (go) delta += ring_level2<FMT>(w, ring0, eoff, lat, tbl);
+                return;
+            }
             const uint32_t mk = __ballot_sync(0xFFFFFFFFu, go);
             if (go) q2[(h2 + n2 + __popc(mk & lt)) & (kRingQ2Cap - 1)] = w;
             if (n_old) {
@@ -412,9 +423,9 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
         if (e != cudaSuccess) return (int)e;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 1024);
+        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 1024);
+        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
         if (e != cudaSuccess) return (int)e;
         sm_count = sms;
     }
@@ -442,8 +453,8 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
     if (const char* e = getenv("PGG_RING_SLOTS")) want = (uint32_t)atoi(e);
     if (want > (uint32_t)kRingMaxSlots) want = kRingMaxSlots;
     if (want < 3) want = 3;
-    const uint32_t fixed = (uint32_t)kRingFixedBytes + 3 * p->pitch;
-    while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 1024) --want;
+    const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes) + 3 * p->pitch;
+    while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 256) --want;
     if (max_chunks < want) want = max_chunks < 3 ? 3 : max_chunks;
     p->NS = want;
     p->smem_bytes = p->NS * p->slot_bytes + fixed;
