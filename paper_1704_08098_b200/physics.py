@@ -1,0 +1,115 @@
+"""Observables of the paper measured with libpgg (GPU only; thin drivers around pgg_run_ensemble).
+
+    python -m paper_1704_08098_b200.physics stationary [--L 400] [--mcs 20000] [--seeds 101 102 103 104]
+                                                       [--order iid|perm] [--rs 3.6 3.65 ...]
+    python -m paper_1704_08098_b200.physics decay --r 3.7443 [--L 2048] [--mcs 100000] [--seeds 1..16]
+
+``stationary``: rho_C(r) of BASELINE.json configs[1] -- the time average of Eq. (4) over
+the second half of the run, with the standard error from 10 batch means, per (r, seed) and pooled.
+``decay``: rho_C(t) of configs[2] averaged over seeds on log-spaced t, and the local decay exponent
+delta_eff(t) = -ln[rho(t)/rho(t/8)] / ln 8 (directed percolation: delta = 0.4505; PAPER.md:97,111 place
+the transition in that class).  Every number comes from the integer count traces the kernels produce;
+the arithmetic here is averaging only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+
+import numpy as np
+
+from . import (FMT_U8, ORDER_IID, ORDER_PERM, pgg_run_ensemble)
+
+
+def run_traces(L, rs, seeds, K, rho0, n_mcs, order=ORDER_IID, fmt=FMT_U8, chunk=None):
+    """One lattice per (r, seed) pair in one ensemble launch -> counts [B, n_mcs] (numpy int64)."""
+    import torch
+    B = len(rs)
+    shape = (B, L, L) if fmt == FMT_U8 else (B, L, L // 32)
+    d = torch.empty(shape, dtype=torch.uint8 if fmt == FMT_U8 else torch.int32, device="cuda")
+    cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+    pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, order, rho0, 0, n_mcs, cnt)
+    torch.cuda.synchronize()
+    return cnt.cpu().numpy()
+
+
+def window_stats(counts, sites, n_batches=10):
+    w = counts[len(counts) // 2:].astype(np.float64) / sites
+    b = w[: len(w) // n_batches * n_batches].reshape(n_batches, -1).mean(axis=1)
+    return float(w.mean()), float(b.std(ddof=1) / math.sqrt(n_batches))
+
+
+def stationary(rs, seeds, L=400, n_mcs=20000, K=0.5, rho0=0.5, order=ORDER_IID):
+    """-> {r: {"per_seed": [(mean, stderr)...], "mean": m, "stderr": e}}; e combines the batch-mean
+    errors with the scatter between seeds (whichever is larger)."""
+    pairs = [(r, s) for r in rs for s in seeds]
+    tr = run_traces(L, [p[0] for p in pairs], [p[1] for p in pairs], K, rho0, n_mcs, order)
+    out = {}
+    for a, r in enumerate(rs):
+        st = [window_stats(tr[a * len(seeds) + b], L * L) for b in range(len(seeds))]
+        means = np.array([m for m, _ in st])
+        within = math.sqrt(sum(e * e for _, e in st)) / len(st)
+        between = float(means.std(ddof=1) / math.sqrt(len(st))) if len(st) > 1 else 0.0
+        out[r] = {"per_seed": st, "mean": float(means.mean()), "stderr": max(within, between)}
+    return out
+
+
+def log_times(n_mcs, per_decade=8):
+    ts, t = set(), 1.0
+    while t <= n_mcs:
+        ts.add(int(t))
+        t *= 10 ** (1.0 / per_decade)
+    ts.add(n_mcs)
+    return sorted(ts)
+
+
+def decay(r, seeds, L=2048, n_mcs=100000, K=0.5, rho0=0.5, order=ORDER_IID):
+    """-> list of rows {t, rho, rho_err, delta_eff, delta_err}: seed average of rho_C(t), error from the
+    scatter between seeds; delta_eff(t) between t/8 and t with a seed-jackknife error."""
+    tr = run_traces(L, [r] * len(seeds), seeds, K, rho0, n_mcs, order).astype(np.float64) / (L * L)
+    rows = []
+    n = len(seeds)
+    for t in log_times(n_mcs):
+        col = tr[:, t - 1]
+        row = {"t": t, "alive": int((col > 0).sum()), "rho": float(col.mean()), "rho_err": float(col.std(ddof=1) / math.sqrt(n)) if n > 1 else 0.0}
+        t8 = t // 8
+        if t8 >= 1 and col.mean() > 0 and tr[:, t8 - 1].mean() > 0:
+            def d_eff(sel):
+                a, b = tr[sel, t - 1].mean(), tr[sel, t8 - 1].mean()
+                return -math.log(a / b) / math.log(t / t8) if a > 0 and b > 0 else float("nan")
+            full = d_eff(slice(None))
+            if n > 1:
+                jk = np.array([d_eff([i for i in range(n) if i != j]) for j in range(n)])
+                err = float(math.sqrt((n - 1) / n * ((jk - jk.mean()) ** 2).sum()))
+            else:
+                err = 0.0
+            row.update(delta_eff=full, delta_err=err)
+        rows.append(row)
+    return rows
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("what", choices=["stationary", "decay"])
+    ap.add_argument("--L", type=int, default=0)
+    ap.add_argument("--mcs", type=int, default=0)
+    ap.add_argument("--seeds", type=int, nargs="+", default=None)
+    ap.add_argument("--order", default="iid", choices=["iid", "perm"])
+    ap.add_argument("--rs", type=float, nargs="+", default=None)
+    ap.add_argument("--r", type=float, default=3.7443)
+    args = ap.parse_args()
+    order = ORDER_IID if args.order == "iid" else ORDER_PERM
+    if args.what == "stationary":
+        rs = args.rs or [round(3.60 + 0.05 * a, 2) for a in range(9)] + [5.3, 5.4, 5.5, 5.6]
+        res = stationary(rs, args.seeds or [101, 102, 103, 104], args.L or 400, args.mcs or 20000, order=order)
+        print(json.dumps({"what": "stationary", "order": args.order, "L": args.L or 400, "mcs": args.mcs or 20000,
+                          "rows": [{"r": r, **v} for r, v in res.items()]}))
+    else:
+        rows = decay(args.r, args.seeds or list(range(1, 17)), args.L or 2048, args.mcs or 100000, order=order)
+        print(json.dumps({"what": "decay", "order": args.order, "r": args.r, "L": args.L or 2048,
+                          "mcs": args.mcs or 100000, "rows": rows}))
+
+
+if __name__ == "__main__":
+    main()
