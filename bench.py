@@ -32,7 +32,7 @@ from pathlib import Path
 ROOT = Path(__file__).resolve().parent
 sys.path.insert(0, str(ROOT))
 
-R, K_NOISE, RHO0, SEED = 3.8, 0.5, 0.5, 1           # BASELINE.json configs[4]
+R, K_NOISE, RHO0, SEED = 3.8, 0.5, 0.5, 1           # BASELINE.json configs[4]; --rho0 overrides RHO0 (profiling aid)
 METRIC = "elementary strategy updates/sec at L=16384"
 
 
@@ -99,6 +99,22 @@ def oracle_sample(L: int, max_mcs: int, min_seconds: float):
             break
     dt = time.perf_counter() - t0
     return done * L * L / dt, threads, done, dt
+
+
+def max_over_ranks(vals, world, device="cpu"):
+    """Timings are reported as the MAX over ranks (the job is as slow as its slowest replica)."""
+    if world == 1:
+        return list(vals)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(vals), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def job_value(world, steps, updates_per_step, ms):
+    """Whole-job throughput: the updates all ranks processed / the slowest rank's time."""
+    return world * steps * updates_per_step / (ms * 1e-3)
 
 
 def run_reference(args):
@@ -206,12 +222,9 @@ def run_ours(args):
     total_ms = ev_a[0].elapsed_time(ev_c[-1])
     sweep_ms = sum(ev_b[i].elapsed_time(ev_c[i]) for i in range(args.steps))
     last_counts = d_counts.cpu()
-    if world > 1:
-        t = torch.tensor([total_ms, sweep_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, sweep_ms = t.tolist()
+    total_ms, sweep_ms = max_over_ranks([total_ms, sweep_ms], world, "cuda")
     updates_per_step = float(n_mcs) * L * L
-    value = world * args.steps * updates_per_step / (total_ms * 1e-3)
+    value = job_value(world, args.steps, updates_per_step, total_ms)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): per step copy the initial
     # lattice host->device, sweep, copy the final lattice and the count trace device->host.
@@ -240,11 +253,8 @@ def run_ours(args):
     barrier()
     e2e_ms = max(e0.elapsed_time(e1), 0.0)
     e2e_wall_ms = (time.perf_counter() - t0) * 1e3
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = t.item()
-    e2e_value = world * e2e_steps * updates_per_step / (e2e_ms * 1e-3)
+    (e2e_ms,) = max_over_ranks([e2e_ms], world, "cuda")
+    e2e_value = job_value(world, e2e_steps, updates_per_step, e2e_ms)
     assert torch.equal(h_counts, last_counts), "e2e run and device-resident run disagree"
 
     if rank != 0:
@@ -320,7 +330,11 @@ def main():
     ap.add_argument("--profile-mcs", type=int, default=-1,
                     help="profiling aid: bracket this MCS with cudaProfilerStart/Stop (ncu --profile-from-start off); "
                          "the run's numbers are then not bench values")
+    ap.add_argument("--rho0", type=float, default=RHO0,
+                    help="initial cooperator fraction; 0 gives an all-D lattice (no site ever needs a draw): the "
+                         "pure streaming rate of the phase kernel.  Anything but 0.5 is not the bench workload")
     args = ap.parse_args()
+    globals()["RHO0"] = args.rho0
     if args.impl == "reference":
         run_reference(args)
     else:
