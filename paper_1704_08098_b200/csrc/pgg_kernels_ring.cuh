@@ -9,10 +9,12 @@
 // generic (parity, ring row, column) queue entries, and the ring-wrap fix-up of
 // every stencil access.  RING removes that work:
 //
-//   * the three lattice rows above ring slot 0 are staged a second time, in
-//     front of slot 0 ("mirror rows", by the same bulk-async copies, counted on
-//     the same mbarrier), so a stencil never wraps inside the ring: every access
-//     is ring0[soff + constant];
+//   * a stencil access is ring0[soff + constant]; only sites in ring row 0 (one
+//     step in NS) can reach above the ring, and only they take a second copy of
+//     the stencil code whose negative offsets get the ring size added.  (The
+//     alternative, PGG_RING_MIRROR=1, stages the three rows above slot 0 a second
+//     time in front of it -- no wrap at all, but 24 KB that a sixth ring slot
+//     uses better: 65.0 -> 63.5 us per launch, profiles/r1_ring_design_notes.md);
 //   * queue entries are self-contained: Q1 = (soff, site), Q2 = (soff|dir|s_x,
 //     site, u); soff = offset of x from ring0 in site units (bytes for uint8,
 //     bits for bit-packed), site = lattice site index (the Philox counter and
@@ -70,6 +72,7 @@ struct RingPlan {
     uint32_t n_groups;   // L / 4 active rows per class
     uint32_t n_super;    // steps per strip = ceil(n_groups / R)
     uint32_t smem_bytes;
+    uint32_t mirror;     // 1: three mirror rows in front of slot 0; 0: wrapping stencil reads
 };
 
 // s at offset `off` (site units) from ring0; off may reach into the mirror rows (< 0)
@@ -80,38 +83,56 @@ __device__ __forceinline__ int ring_get(const uint8_t* ring0, int off)
     return (ring0[off >> 3] >> (off & 7)) & 1;
 }
 
+// Without mirror rows a read above ring row 0 lands at the end of the ring: `wrap` = ring size in
+// site units is added to a negative offset.
+template <int FMT>
+__device__ __forceinline__ int ring_getw(const uint8_t* ring0, int off, int wrap)
+{
+    return ring_get<FMT>(ring0, off + ((off >> 31) & wrap));
+}
+
 // Level 1 (a3, a4): draw, neighbour compare.  Returns true if the site goes on to level 2.
 template <int FMT>
 __device__ __forceinline__ bool ring_level1(uint2 e, const uint8_t* ring0, const int* __restrict__ eoff,
-                                            const StepKey& sk, uint4& out)
+                                            const StepKey& sk, uint4& out, int wrap)
 {
     uint32_t x0, u;
     step_draw(sk, e.y, x0, u);
     const uint32_t dir = x0 >> 30;  // 0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1)
     const int soff = (int)e.x;
     const int sx = ring_get<FMT>(ring0, soff);
-    const int sy = ring_get<FMT>(ring0, soff + eoff[dir]);
+    const int sy = ring_getw<FMT>(ring0, soff + eoff[dir], wrap);  // wrap == 0 with mirror rows
     out = make_uint4(e.x | (dir << 30) | ((uint32_t)sx << 29), e.y, u, 0u);
     return sx != sy;
 }
 
 // Level 2 (a5-a7): payoff difference, acceptance, write.  Returns the change of the cooperator count.
+template <int FMT, bool WRAP>
+__device__ __forceinline__ int ring_stencil(int soff, uint32_t dir, int sx, const uint8_t* ring0,
+                                            const int* __restrict__ eoff, int wrap)
+{
+    // e = step towards y, f = perpendicular step (site units)
+    const int e = eoff[dir], f = eoff[4 + dir], f2 = 2 * f;
+    const int pm1 = soff - e, pm2 = pm1 - e, p1 = soff + e, p2 = p1 + e, p3 = p2 + e;
+    auto G = [&](int off) { return WRAP ? ring_getw<FMT>(ring0, off, wrap) : ring_get<FMT>(ring0, off); };
+    // A_x - A_y with A = 5 s + 2 (nearest + diagonal) + axial distance-2 (include/pgg.h):
+    // weights of x's 13-site stencil minus those of y's, y = x + e; s_x - s_y = 2 s_x - 1
+    return G(pm2) + G(pm1) - G(p2) - G(p3) + 3 * (2 * sx - 1)
+         + 2 * (G(pm1 + f) + G(pm1 - f) - G(p2 + f) - G(p2 - f))
+         + G(soff + f2) + G(soff - f2) - G(p1 + f2) - G(p1 - f2);
+}
+
+// `wrap_below`: sites with soff below it (ring row 0) take the wrapping stencil; 0 with mirror rows.
 template <int FMT>
 __device__ __forceinline__ int ring_level2(uint4 w, const uint8_t* ring0, const int* __restrict__ eoff,
-                                           uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl)
+                                           uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl,
+                                           int wrap, int wrap_below)
 {
     const int soff = (int)(w.x & 0x1FFFFFFFu);
     const uint32_t dir = w.x >> 30;
     const int sx = (int)((w.x >> 29) & 1u);
-    // e = step towards y, f = perpendicular step (site units)
-    const int e = eoff[dir], f = eoff[4 + dir], f2 = 2 * f;
-    const int pm1 = soff - e, pm2 = pm1 - e, p1 = soff + e, p2 = p1 + e, p3 = p2 + e;
-    auto G = [&](int off) { return ring_get<FMT>(ring0, off); };
-    // A_x - A_y with A = 5 s + 2 (nearest + diagonal) + axial distance-2 (include/pgg.h):
-    // weights of x's 13-site stencil minus those of y's, y = x + e; s_x - s_y = 2 s_x - 1
-    const int dA = G(pm2) + G(pm1) - G(p2) - G(p3) + 3 * (2 * sx - 1)
-                 + 2 * (G(pm1 + f) + G(pm1 - f) - G(p2 + f) - G(p2 - f))
-                 + G(soff + f2) + G(soff - f2) - G(p1 + f2) - G(p1 - f2);
+    const int dA = soff < wrap_below ? ring_stencil<FMT, true>(soff, dir, sx, ring0, eoff, wrap)
+                                     : ring_stencil<FMT, false>(soff, dir, sx, ring0, eoff, 0);
     // table_index(dA, ds) = (ds + 1) * 51 + dA + 25 with ds = 2 s_x - 1
     if (w.z < tbl[sx * 102 + dA + 25]) {
         if (FMT == kFmtU8)
@@ -130,7 +151,8 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const uint32_t NS = g.NS;
     const int RC = (int)g.RC, pitch = (int)g.pitch;
-    uint8_t* ring0 = smem_raw + 3 * pitch;  // three mirror rows in front of slot 0
+    const bool use_mirror = g.mirror != 0;
+    uint8_t* ring0 = smem_raw + (use_mirror ? 3 * pitch : 0);  // three mirror rows in front of slot 0
     uint8_t* qbase = ring0 + (size_t)NS * g.slot_bytes;
     uint32_t* tbl = reinterpret_cast<uint32_t*>(qbase + kRingConsumers * RingCfg<FMT>::warp_q_bytes);
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(tbl + 160);  // full[NS], empty[NS]
@@ -182,7 +204,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
             if (use > 0) mbar_wait(bar_empty + 8u * slot, (use - 1u) & 1u);
             const uint32_t bar = bar_full + 8u * slot;
             const int r_lo = kc == 0 ? RC - 3 : 0;  // of the prologue chunk only the tail is read
-            const bool mirror = slot == NS - 1;     // its last three rows are also staged above slot 0
+            const bool mirror = use_mirror && slot == NS - 1;     // its last three rows are also staged above slot 0
             if (lane == 0) mbar_expect_tx(bar, (uint32_t)(RC - r_lo + (mirror ? 3 : 0)) * row_tx);
             __syncwarp();
             for (int q = r_lo + lane; q < RC + (mirror ? 3 : 0); q += 32) {
@@ -220,6 +242,10 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         const bool in = colb < wb;
         const int slot_bytes = (int)g.slot_bytes;
         const int ring_bytes = (int)NS * slot_bytes;
+        // site units; both 0 with mirror rows (then no read ever wraps)
+        const int ps_sites = (FMT == kFmtU8) ? pitch : 8 * pitch;
+        const int wrap = use_mirror ? 0 : ((FMT == kFmtU8) ? ring_bytes : 8 * ring_bytes);
+        const int wrap_below = use_mirror ? 0 : ps_sites;
         // Q1 is linear, entries [0, n1); Q2 is a ring of kRingQ2Cap entries, [h2, h2 + n2).
         // o1 / o2 = how many entries at the front were queued by the previous step (they
         // must be finished before this step ends, when their rows are released).
@@ -231,6 +257,9 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         // this lane's 16 bytes of the warp's active row: byte offset from ring0, and the
         // lattice site index of the first of them
         int rowoff = (int)slot * slot_bytes + 4 * rho * pitch + kRingHaloB + colb;
+        // byte offset from this lane's 16 bytes to the same columns one lattice row up
+        const int up_wrapped = (use_mirror || rho != 0) ? -pitch : ring_bytes - pitch;
+        int upoff = (slot == 0) ? up_wrapped : -pitch;
         uint32_t site0 = (uint32_t)(RC * (int)S0 + 4 * rho + ci) * L
                        + (uint32_t)((FMT == kFmtU8) ? j0b + colb : 8 * (j0b + colb));
         const uint32_t site_step = (uint32_t)RC * L;
@@ -242,7 +271,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         // level 2 on the first `cnt` (<= 32) entries of Q2
         auto run_level2 = [&](uint32_t cnt) {
             if ((uint32_t)lane < cnt)
-                delta += ring_level2<FMT>(q2[(h2 + lane) & (kRingQ2Cap - 1)], ring0, eoff, lat, tbl);
+                delta += ring_level2<FMT>(q2[(h2 + lane) & (kRingQ2Cap - 1)], ring0, eoff, lat, tbl, wrap, wrap_below);
             __syncwarp();  // entries are read before a later append may overwrite them
             h2 += cnt;
             n2 -= cnt;
@@ -251,7 +280,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         // Q2 append of one level-1 batch whose first `n_old` lanes hold old entries
         auto push2 = [&](bool go, const uint4& w, uint32_t n_old) {
             if (!RingCfg<FMT>::q2) {
-                if (go) delta += ring_level2<FMT>(w, ring0, eoff, lat, tbl);
+                if (go) delta += ring_level2<FMT>(w, ring0, eoff, lat, tbl, wrap, wrap_below);
                 return;
             }
             const uint32_t mk = __ballot_sync(0xFFFFFFFFu, go);
@@ -268,7 +297,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         auto run_level1 = [&](uint32_t head, uint32_t cnt, uint32_t n_old) {
             uint4 w;
             bool go = false;
-            if ((uint32_t)lane < cnt) go = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, w);
+            if ((uint32_t)lane < cnt) go = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, w, wrap);
             push2(go, w, n_old);
         };
         // full batches from the front of Q1 (two at a time while 64 wait); the leftover
@@ -279,8 +308,8 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
             if (n1 >= 64u) {
                 do {
                     uint4 wa, wb2;
-                    const bool ga = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, wa);
-                    const bool gb = ring_level1<FMT>(q1[head + 32 + lane], ring0, eoff, sk, wb2);
+                    const bool ga = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, wa, wrap);
+                    const bool gb = ring_level1<FMT>(q1[head + 32 + lane], ring0, eoff, sk, wb2, wrap);
                     push2(ga, wa, head ? 0u : o1);
                     push2(gb, wb2, 0u);
                     head += 64u;
@@ -312,7 +341,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
                 uint32_t pv = 0, nx = 0;
                 if (in) {
                     wc = *reinterpret_cast<const uint4*>(rowp);
-                    wu = *reinterpret_cast<const uint4*>(rowp - pitch);
+                    wu = *reinterpret_cast<const uint4*>(rowp + upoff);
                     wd = *reinterpret_cast<const uint4*>(rowp + pitch);
                     pv = *reinterpret_cast<const uint32_t*>(rowp - 4);
                     nx = *reinterpret_cast<const uint32_t*>(rowp + 16);
@@ -385,7 +414,8 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
             o2 = n2;
             site0 += site_step;
             rowoff += slot_bytes;
-            if (++slot == NS) { slot = 0; par ^= 1u; rowoff -= ring_bytes; }
+            upoff = -pitch;
+            if (++slot == NS) { slot = 0; par ^= 1u; rowoff -= ring_bytes; upoff = up_wrapped; }
         }
         // drain: everything left was queued by the last step
         if (n1) {
@@ -453,7 +483,10 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
     if (const char* e = getenv("PGG_RING_SLOTS")) want = (uint32_t)atoi(e);
     if (want > (uint32_t)kRingMaxSlots) want = kRingMaxSlots;
     if (want < 3) want = 3;
-    const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes) + 3 * p->pitch;
+    p->mirror = 0;
+    if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = atoi(e) ? 1u : 0u;
+    const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
+                         + (p->mirror ? 3 * p->pitch : 0);
     while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 256) --want;
     if (max_chunks < want) want = max_chunks < 3 ? 3 : max_chunks;
     p->NS = want;
