@@ -19,6 +19,7 @@
 #include "pgg_kernels_pipe.cuh"
 #include "pgg_kernels_band.cuh"
 #include "pgg_kernels_ring.cuh"
+#include "pgg_kernels_split.cuh"
 
 namespace {
 
@@ -144,7 +145,9 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     const bool band_ok = pgg::band_supported(fmt, L);
     const bool ring_ok = pgg::ring_supported(fmt, L);
     if (variant == PGG_VARIANT_AUTO) variant = ring_ok ? PGG_VARIANT_RING : PGG_VARIANT_V0;
-    if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok))
+    const bool split_ok = pgg::split_supported(fmt, L);
+    if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
+        (variant == PGG_VARIANT_SPLIT && !split_ok))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_FUSED || variant == PGG_VARIANT_PIPE) && !tile_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
@@ -202,6 +205,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     pgg::TilePlan plan;
     pgg::BandPlan bplan;
     pgg::RingPlan rplan;
+    if (variant == PGG_VARIANT_SPLIT) {
+        int32_t rc = pgg::split_plan(L, B, &rplan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "split kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
     if (variant == PGG_VARIANT_RING) {
         int32_t rc = pgg::ring_plan(fmt, L, B, &rplan);
         if (rc != 0) return fail(PGG_ERR_CUDA, "ring kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
@@ -226,7 +233,9 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         PGG_LAUNCHED();
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
-                if (variant == PGG_VARIANT_RING) {
+                if (variant == PGG_VARIANT_SPLIT) {
+                    pgg::split_launch(rplan, a, m, k, B, stream);
+                } else if (variant == PGG_VARIANT_RING) {
                     pgg::ring_launch(rplan, fmt, a, m, k, B, stream);
                 } else if (variant == PGG_VARIANT_BAND) {
                     pgg::band_launch(bplan, fmt, a, m, k, B, stream);
@@ -345,7 +354,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_RING)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_SPLIT)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -361,6 +370,7 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_PIPE) return pgg::tile_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_BAND) return pgg::band_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_RING) return pgg::ring_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_SPLIT) return pgg::split_supported(fmt, L) ? 1 : 0;
     return 0;
 }
 
