@@ -73,7 +73,8 @@ enum {
     PGG_VARIANT_PIPE = 4, /* TILE staging as a producer/consumer warp pipeline        */
     PGG_VARIANT_BAND = 5, /* row bands of wide strips streamed through a smem ring    */
     PGG_VARIANT_RING = 6, /* BAND's data movement, consumer cut to the fewest instr.  */
-    PGG_VARIANT_SPLIT = 7 /* RING with scanner and worker warps (uint8 only)          */
+    PGG_VARIANT_SPLIT = 7,/* RING with scanner and worker warps (uint8 only)          */
+    PGG_VARIANT_DYN = 8   /* RING with dynamically assigned tasks, 24 warps (uint8)   */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:

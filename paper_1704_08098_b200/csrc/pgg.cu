@@ -20,6 +20,7 @@
 #include "pgg_kernels_band.cuh"
 #include "pgg_kernels_ring.cuh"
 #include "pgg_kernels_split.cuh"
+#include "pgg_kernels_dyn.cuh"
 
 namespace {
 
@@ -147,7 +148,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     if (variant == PGG_VARIANT_AUTO) variant = ring_ok ? PGG_VARIANT_RING : PGG_VARIANT_V0;
     const bool split_ok = pgg::split_supported(fmt, L);
     if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
-        (variant == PGG_VARIANT_SPLIT && !split_ok))
+        (variant == PGG_VARIANT_SPLIT && !split_ok) || (variant == PGG_VARIANT_DYN && !pgg::dyn_supported(fmt, L)))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_FUSED || variant == PGG_VARIANT_PIPE) && !tile_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
@@ -205,6 +206,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     pgg::TilePlan plan;
     pgg::BandPlan bplan;
     pgg::RingPlan rplan;
+    if (variant == PGG_VARIANT_DYN) {
+        int32_t rc = pgg::dyn_plan(L, B, &rplan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "dyn kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
     if (variant == PGG_VARIANT_SPLIT) {
         int32_t rc = pgg::split_plan(L, B, &rplan);
         if (rc != 0) return fail(PGG_ERR_CUDA, "split kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
@@ -233,7 +238,9 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         PGG_LAUNCHED();
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
-                if (variant == PGG_VARIANT_SPLIT) {
+                if (variant == PGG_VARIANT_DYN) {
+                    pgg::dyn_launch(rplan, a, m, k, B, stream);
+                } else if (variant == PGG_VARIANT_SPLIT) {
                     pgg::split_launch(rplan, a, m, k, B, stream);
                 } else if (variant == PGG_VARIANT_RING) {
                     pgg::ring_launch(rplan, fmt, a, m, k, B, stream);
@@ -354,7 +361,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_SPLIT)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_DYN)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -371,6 +378,7 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_BAND) return pgg::band_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_RING) return pgg::ring_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_SPLIT) return pgg::split_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_DYN) return pgg::dyn_supported(fmt, L) ? 1 : 0;
     return 0;
 }
 

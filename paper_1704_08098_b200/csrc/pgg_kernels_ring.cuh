@@ -144,7 +144,9 @@ __device__ __forceinline__ int ring_level2(uint4 w, const uint8_t* ring0, const 
     return 0;
 }
 
-template <int FMT>
+// FULL: every strip is W bytes wide and every warp has an active row in every step (no ragged
+// edges: the per-lane and per-step guards of the scan drop out).
+template <int FMT, bool FULL>
 __global__ void __launch_bounds__(kRingThreads, 1)
 phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
 {
@@ -162,11 +164,14 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
     const uint32_t b = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t L = a.L;
-    const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
-    const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
     const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8u * NS;
 
+    // Programmatic dependent launch: the next phase's CTAs may take an SM as soon as this
+    // kernel's CTA there has exited, and set themselves up; they touch nothing a previous
+    // kernel wrote (the lattice, the phase order) before griddepcontrol.wait returns, i.e.
+    // before the whole previous grid has completed and its writes are visible.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (int q = threadIdx.x; q < kTableSize; q += kRingThreads)
         tbl[q] = a.tables[(size_t)b * kTableSize + q];
     if (threadIdx.x == 0) {
@@ -181,6 +186,9 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         eoff[4] = 1;   eoff[5] = 1;  eoff[6] = ps; eoff[7] = ps;
     }
     __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
+    const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
 
     const uint32_t strip = blockIdx.x / g.nb, band = blockIdx.x - strip * g.nb;
     const uint32_t S0 = (uint32_t)(((unsigned long long)band * g.n_super) / g.nb);
@@ -335,11 +343,11 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         if (n_steps) mbar_wait(bar_full, 0u);
         for (uint32_t s = 0; s < n_steps; ++s) {
             mbar_wait(bar_full + 8u * slot, par);
-            if (s < n_act) {
+            if (FULL || s < n_act) {
                 const uint8_t* rowp = ring0 + rowoff;
                 uint4 wc = make_uint4(0, 0, 0, 0), wu = wc, wd = wc;
                 uint32_t pv = 0, nx = 0;
-                if (in) {
+                if (FULL || in) {
                     wc = *reinterpret_cast<const uint4*>(rowp);
                     wu = *reinterpret_cast<const uint4*>(rowp + upoff);
                     wd = *reinterpret_cast<const uint4*>(rowp + pitch);
@@ -405,7 +413,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
                 run_level1(0u, n1, o1);
                 n1 = 0;
             }
-            if (o2) run_level2(n2);  // then n2 < 32
+            if (RingCfg<FMT>::q2 && o2) run_level2(n2);  // then n2 < 32
             if (s > 0) {
                 if (lane == 0) mbar_arrive(bar_empty + 8u * rel_slot);  // chunk s-1 is free
                 if (++rel_slot == NS) rel_slot = 0;
@@ -453,9 +461,13 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
         if (e != cudaSuccess) return (int)e;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+        if (e != cudaSuccess) return (int)e;
+        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+        if (e != cudaSuccess) return (int)e;
+        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
         if (e != cudaSuccess) return (int)e;
         sm_count = sms;
     }
@@ -497,11 +509,25 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
 inline void ring_launch(const RingPlan& p, int fmt, const PhaseArgs& a, uint32_t m, uint32_t k,
                         uint32_t B, cudaStream_t stream)
 {
-    dim3 grid(p.n_strips * p.nb, B);
-    if (fmt == kFmtU8)
-        phase_ring_kernel<kFmtU8><<<grid, kRingThreads, p.smem_bytes, stream>>>(a, m, k, p);
-    else
-        phase_ring_kernel<kFmtBits><<<grid, kRingThreads, p.smem_bytes, stream>>>(a, m, k, p);
+    static const bool pdl = [] { const char* e = getenv("PGG_PDL"); return e == nullptr || atoi(e) != 0; }();
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.n_strips * p.nb, B);
+    cfg.blockDim = dim3(kRingThreads);
+    cfg.dynamicSmemBytes = p.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const bool full = p.row_bytes % p.W == 0 && p.n_groups % p.R == 0;
+    if (fmt == kFmtU8) {
+        if (full) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, true>, a, m, k, p);
+        else cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, false>, a, m, k, p);
+    } else {
+        if (full) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, true>, a, m, k, p);
+        else cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, false>, a, m, k, p);
+    }
 }
 
 }  // namespace pgg
