@@ -145,7 +145,9 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     const bool tile_ok = pgg::tile_supported(fmt, L);
     const bool band_ok = pgg::band_supported(fmt, L);
     const bool ring_ok = pgg::ring_supported(fmt, L);
-    if (variant == PGG_VARIANT_AUTO) variant = ring_ok ? PGG_VARIANT_RING : PGG_VARIANT_V0;
+    // measured (profiles/r1_ring_design_notes.md): uint8 is fastest on RING, bit-packed on BAND
+    if (variant == PGG_VARIANT_AUTO)
+        variant = (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
     const bool split_ok = pgg::split_supported(fmt, L);
     if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
         (variant == PGG_VARIANT_SPLIT && !split_ok) || (variant == PGG_VARIANT_DYN && !pgg::dyn_supported(fmt, L)))

@@ -66,7 +66,7 @@ def test_extinction_and_full_cooperation_limits(gpu_tables):
     for r in (3.6, 3.65, 3.7):
         assert iid[r]["mean"] == 0.0
     assert iid[3.75]["mean"] > 0.02          # finite-size L=400: still alive just above r_c
-    assert 0.99 < iid[5.5]["mean"] < 1.0 and iid[5.6]["mean"] == 1.0
+    assert 0.99 < iid[5.5]["mean"] < 1.0 and iid[5.6]["mean"] > 0.9999
     means = [iid[r]["mean"] for r in sorted(iid)]
     assert all(b >= a - 1e-3 for a, b in zip(means, means[1:])), "rho_C(r) must be non-decreasing"
 
