@@ -124,24 +124,51 @@ __device__ __forceinline__ int ring_stencil(int soff, uint32_t dir, int sx, cons
 
 // `wrap_below`: sites with soff below it (ring row 0) take the wrapping stencil; 0 with mirror rows.
 template <int FMT>
+__device__ __forceinline__ int ring_accept(int soff, uint32_t dir, int sx, uint32_t site, uint32_t u,
+                                           const uint8_t* ring0, const int* __restrict__ eoff,
+                                           uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl,
+                                           int wrap, int wrap_below)
+{
+    const int dA = soff < wrap_below ? ring_stencil<FMT, true>(soff, dir, sx, ring0, eoff, wrap)
+                                     : ring_stencil<FMT, false>(soff, dir, sx, ring0, eoff, 0);
+    // table_index(dA, ds) = (ds + 1) * 51 + dA + 25 with ds = 2 s_x - 1
+    if (u < tbl[sx * 102 + dA + 25]) {
+        if (FMT == kFmtU8)
+            lat[site] = (uint8_t)(1 - sx);
+        else
+            atomicXor(reinterpret_cast<uint32_t*>(lat) + (site >> 5), 1u << (site & 31u));
+        return 1 - 2 * sx;
+    }
+    return 0;
+}
+
+// Level 2 on a Q2 entry (soff | dir << 30 | s_x << 29, site, u)
+template <int FMT>
 __device__ __forceinline__ int ring_level2(uint4 w, const uint8_t* ring0, const int* __restrict__ eoff,
                                            uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl,
                                            int wrap, int wrap_below)
 {
-    const int soff = (int)(w.x & 0x1FFFFFFFu);
-    const uint32_t dir = w.x >> 30;
-    const int sx = (int)((w.x >> 29) & 1u);
-    const int dA = soff < wrap_below ? ring_stencil<FMT, true>(soff, dir, sx, ring0, eoff, wrap)
-                                     : ring_stencil<FMT, false>(soff, dir, sx, ring0, eoff, 0);
-    // table_index(dA, ds) = (ds + 1) * 51 + dA + 25 with ds = 2 s_x - 1
-    if (w.z < tbl[sx * 102 + dA + 25]) {
-        if (FMT == kFmtU8)
-            lat[w.y] = (uint8_t)(1 - sx);
-        else
-            atomicXor(reinterpret_cast<uint32_t*>(lat) + (w.y >> 5), 1u << (w.y & 31u));
-        return 1 - 2 * sx;
-    }
-    return 0;
+    return ring_accept<FMT>((int)(w.x & 0x1FFFFFFFu), w.x >> 30, (int)((w.x >> 29) & 1u), w.y, w.z, ring0, eoff,
+                            lat, tbl, wrap, wrap_below);
+}
+
+// Levels 1 and 2 of one queued site without the Q2 entry in between (the inline path)
+struct RingDraw {
+    uint32_t dir, u;
+    int sx;
+    bool go;
+};
+template <int FMT>
+__device__ __forceinline__ RingDraw ring_draw(uint2 e, const uint8_t* ring0, const int* __restrict__ eoff,
+                                              const StepKey& sk, int wrap)
+{
+    RingDraw d;
+    uint32_t x0;
+    step_draw(sk, e.y, x0, d.u);
+    d.dir = x0 >> 30;
+    d.sx = ring_get<FMT>(ring0, (int)e.x);
+    d.go = d.sx != ring_getw<FMT>(ring0, (int)e.x + eoff[d.dir], wrap);
+    return d;
 }
 
 // FULL: every strip is W bytes wide and every warp has an active row in every step (no ragged
@@ -303,6 +330,15 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         };
         // level 1 on `cnt` (<= 32) entries of Q1 starting at `head`
         auto run_level1 = [&](uint32_t head, uint32_t cnt, uint32_t n_old) {
+            if (!RingCfg<FMT>::q2) {
+                if ((uint32_t)lane < cnt) {
+                    const uint2 e = q1[head + lane];
+                    const RingDraw d = ring_draw<FMT>(e, ring0, eoff, sk, wrap);
+                    if (d.go)
+                        delta += ring_accept<FMT>((int)e.x, d.dir, d.sx, e.y, d.u, ring0, eoff, lat, tbl, wrap, wrap_below);
+                }
+                return;
+            }
             uint4 w;
             bool go = false;
             if ((uint32_t)lane < cnt) go = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, w, wrap);
@@ -315,6 +351,17 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
             uint32_t head = 0;
             if (n1 >= 64u) {
                 do {
+                    if (!RingCfg<FMT>::q2) {  // two independent Philox chains, then the two stencils
+                        const uint2 ea = q1[head + lane], eb = q1[head + 32 + lane];
+                        const RingDraw da = ring_draw<FMT>(ea, ring0, eoff, sk, wrap);
+                        const RingDraw db = ring_draw<FMT>(eb, ring0, eoff, sk, wrap);
+                        if (da.go)
+                            delta += ring_accept<FMT>((int)ea.x, da.dir, da.sx, ea.y, da.u, ring0, eoff, lat, tbl, wrap, wrap_below);
+                        if (db.go)
+                            delta += ring_accept<FMT>((int)eb.x, db.dir, db.sx, eb.y, db.u, ring0, eoff, lat, tbl, wrap, wrap_below);
+                        head += 64u;
+                        continue;
+                    }
                     uint4 wa, wb2;
                     const bool ga = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, wa, wrap);
                     const bool gb = ring_level1<FMT>(q1[head + 32 + lane], ring0, eoff, sk, wb2, wrap);
