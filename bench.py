@@ -171,7 +171,7 @@ def run_ours(args):
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
                "fused": pgg.VARIANT_FUSED, "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND,
-               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN}[args.variant]
+               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT}[args.variant]
     pgg.pgg_set_variant(variant)
     seed = SEED + rank
     shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
@@ -325,7 +325,7 @@ def main():
     ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
-    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band", "ring", "split", "dyn"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band", "ring", "split", "dyn", "resident"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-mcs", type=int, default=-1,
                     help="profiling aid: bracket this MCS with cudaProfilerStart/Stop (ncu --profile-from-start off); "

@@ -64,7 +64,8 @@ enum { PGG_FMT_U8 = 0, PGG_FMT_BITS = 1 };
 enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1 };
 
 /* Kernel variants of the phase step (all bit-identical).
- * PGG_VARIANT_AUTO picks the fastest one that supports (fmt, L).                 */
+ * PGG_VARIANT_AUTO picks the fastest one that supports (fmt, L): RESIDENT for
+ * L <= 512, else RING (uint8) / BAND (bit-packed), else V0.                       */
 enum {
     PGG_VARIANT_AUTO = 0,
     PGG_VARIANT_V0 = 1,   /* one thread per active site, global loads, any L % 4 == 0 */
@@ -74,7 +75,9 @@ enum {
     PGG_VARIANT_BAND = 5, /* row bands of wide strips streamed through a smem ring    */
     PGG_VARIANT_RING = 6, /* BAND's data movement, consumer cut to the fewest instr.  */
     PGG_VARIANT_SPLIT = 7,/* RING with scanner and worker warps (uint8 only)          */
-    PGG_VARIANT_DYN = 8   /* RING with dynamically assigned tasks, 24 warps (uint8)   */
+    PGG_VARIANT_DYN = 8,  /* RING with dynamically assigned tasks, 24 warps (uint8)   */
+    PGG_VARIANT_RESIDENT = 9 /* L <= 512: one CTA per lattice, lattice resident in smem,
+                                every phase of the call in one launch                  */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:

@@ -21,6 +21,7 @@
 #include "pgg_kernels_ring.cuh"
 #include "pgg_kernels_split.cuh"
 #include "pgg_kernels_dyn.cuh"
+#include "pgg_kernels_resident.cuh"
 
 namespace {
 
@@ -145,9 +146,14 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     const bool tile_ok = pgg::tile_supported(fmt, L);
     const bool band_ok = pgg::band_supported(fmt, L);
     const bool ring_ok = pgg::ring_supported(fmt, L);
-    // measured (profiles/r1_ring_design_notes.md): uint8 is fastest on RING, bit-packed on BAND
+    // measured (profiles/r1_ring_design_notes.md): small lattices stay resident in shared memory;
+    // of the streaming kernels uint8 is fastest on RING, bit-packed on BAND
+    const bool res_ok = pgg::resident_supported(fmt, L);
     if (variant == PGG_VARIANT_AUTO)
-        variant = (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
+        variant = res_ok ? PGG_VARIANT_RESIDENT
+                : (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
+    if (variant == PGG_VARIANT_RESIDENT && !res_ok)
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     const bool split_ok = pgg::split_supported(fmt, L);
     if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
         (variant == PGG_VARIANT_SPLIT && !split_ok) || (variant == PGG_VARIANT_DYN && !pgg::dyn_supported(fmt, L)))
@@ -233,11 +239,21 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         if (rc != 0) return fail(PGG_ERR_CUDA, "tile kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
     }
 
+    pgg::ResPlan resplan;
+    if (variant == PGG_VARIANT_RESIDENT) {
+        int32_t rc = pgg::resident_plan(fmt, L, &resplan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "resident kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
     for (uint32_t m0 = 0; m0 < n_mcs; m0 += chunk) {
         const uint32_t n_chunk = std::min<uint32_t>(chunk, n_mcs - m0);
         pgg::order_kernel<<<(B * n_chunk + 127) / 128, 128, 0, stream>>>(
             d_seeds, B, t_begin + m0, n_chunk, chunk, order_mode, d_order);
         PGG_LAUNCHED();
+        if (variant == PGG_VARIANT_RESIDENT) {  // all 16 * n_chunk phases in one launch
+            pgg::resident_launch(resplan, fmt, a, m0, n_chunk, B, stream);
+            PGG_LAUNCHED();
+            continue;
+        }
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
                 if (variant == PGG_VARIANT_DYN) {
@@ -363,7 +379,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_DYN)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_RESIDENT)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -381,6 +397,7 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_RING) return pgg::ring_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_SPLIT) return pgg::split_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_DYN) return pgg::dyn_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_RESIDENT) return pgg::resident_supported(fmt, L) ? 1 : 0;
     return 0;
 }
 

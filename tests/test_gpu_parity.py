@@ -16,7 +16,8 @@ import paper_1704_08098_b200 as pgg  # noqa: E402
 
 K = wl.K_DEFAULT
 FMTS = [pgg.FMT_U8, pgg.FMT_BITS]
-VARIANTS = [pgg.VARIANT_V0, pgg.VARIANT_TILE, pgg.VARIANT_PIPE, pgg.VARIANT_BAND, pgg.VARIANT_RING, pgg.VARIANT_SPLIT, pgg.VARIANT_DYN]
+VARIANTS = [pgg.VARIANT_V0, pgg.VARIANT_TILE, pgg.VARIANT_PIPE, pgg.VARIANT_BAND, pgg.VARIANT_RING, pgg.VARIANT_SPLIT, pgg.VARIANT_DYN,
+            pgg.VARIANT_RESIDENT]
 
 
 @pytest.fixture(scope="module", autouse=True)
