@@ -59,7 +59,7 @@ sweep_resident_kernel(PhaseArgs a, uint32_t m0, uint32_t n_chunk, ResPlan g)
 
     const uint32_t b = blockIdx.x;
     const int L = (int)a.L, PW = (int)g.PW, PB = 32 * PW;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
     Lattice<FMT> glat{lat, L};
 

@@ -93,3 +93,22 @@ def test_product_does_not_import_the_oracle():
         if p.suffix in {".py", ".c"}:
             assert "import paper_1704_08098_b200" not in p.read_text()
             assert "pgg.h" not in p.read_text()
+
+
+def test_variant_support_table():
+    """pgg_variant_supported is pure host logic: which kernel may run which (fmt, L)."""
+    sup = pgg.pgg_variant_supported
+    for L in (4, 20, 64, 400, 512, 2048, 16384):
+        assert sup(pgg.VARIANT_AUTO, pgg.FMT_U8, L) and sup(pgg.VARIANT_V0, pgg.FMT_U8, L)
+    assert not sup(pgg.VARIANT_V0, pgg.FMT_U8, 6) and not sup(pgg.VARIANT_V0, pgg.FMT_BITS, 48)
+    # smem-resident kernel: 8 <= L <= 512 (bit-packed: L % 32 == 0)
+    assert sup(pgg.VARIANT_RESIDENT, pgg.FMT_U8, 8) and sup(pgg.VARIANT_RESIDENT, pgg.FMT_U8, 400)
+    assert sup(pgg.VARIANT_RESIDENT, pgg.FMT_U8, 512) and sup(pgg.VARIANT_RESIDENT, pgg.FMT_BITS, 512)
+    assert not sup(pgg.VARIANT_RESIDENT, pgg.FMT_U8, 4) and not sup(pgg.VARIANT_RESIDENT, pgg.FMT_U8, 516)
+    # streaming kernels need rows of whole 16-byte units
+    assert sup(pgg.VARIANT_RING, pgg.FMT_U8, 400) and not sup(pgg.VARIANT_RING, pgg.FMT_U8, 100)
+    assert sup(pgg.VARIANT_BAND, pgg.FMT_BITS, 16384) and not sup(pgg.VARIANT_BAND, pgg.FMT_BITS, 160)
+    # SPLIT and DYN are uint8 only
+    assert sup(pgg.VARIANT_SPLIT, pgg.FMT_U8, 2048) and not sup(pgg.VARIANT_SPLIT, pgg.FMT_BITS, 2048)
+    assert sup(pgg.VARIANT_DYN, pgg.FMT_U8, 2048) and not sup(pgg.VARIANT_DYN, pgg.FMT_BITS, 2048)
+    assert not sup(99, pgg.FMT_U8, 64)
