@@ -73,6 +73,7 @@ struct RingPlan {
     uint32_t n_super;    // steps per strip = ceil(n_groups / R)
     uint32_t smem_bytes;
     uint32_t mirror;     // 1: three mirror rows in front of slot 0; 0: wrapping stencil reads
+    uint32_t rotate;     // 1: column tasks rotate over the warps from step to step
 };
 
 // s at offset `off` (site units) from ring0; off may reach into the mirror rows (< 0)
@@ -275,6 +276,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         const int rho = warp >> g.tpr_log2, tau = warp & ((1 << g.tpr_log2) - 1);
         const int colb = tau * kRingTaskB + 16 * lane;  // first core byte of this lane's 16
         const bool in = colb < wb;
+        const bool rotate = FULL && FMT == kFmtU8 && g.tpr_log2 == 4 && g.rotate != 0;
         const int slot_bytes = (int)g.slot_bytes;
         const int ring_bytes = (int)NS * slot_bytes;
         // site units; both 0 with mirror rows (then no read ever wraps)
@@ -390,8 +392,11 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         if (n_steps) mbar_wait(bar_full, 0u);
         for (uint32_t s = 0; s < n_steps; ++s) {
             mbar_wait(bar_full + 8u * slot, par);
+            // ROTATE: warp w takes column task (w + s) mod 16 of step s, so that no warp is tied to
+            // the busiest columns of the band for good (queue entries are self-contained)
+            const int rot = rotate ? ((((warp + (int)s) & 15) - tau) * kRingTaskB) : 0;
             if (FULL || s < n_act) {
-                const uint8_t* rowp = ring0 + rowoff;
+                const uint8_t* rowp = ring0 + rowoff + rot;
                 uint4 wc = make_uint4(0, 0, 0, 0), wu = wc, wd = wc;
                 uint32_t pv = 0, nx = 0;
                 if (FULL || in) {
@@ -415,7 +420,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
                         nb[w] = ((c4[w] ^ u4[w]) | (c4[w] ^ d4[w]) | (c4[w] ^ lw) | (c4[w] ^ rw)) & bm;  // S9
                     }
                     if (__any_sync(0xFFFFFFFFu, (nb[0] | nb[1] | nb[2] | nb[3]) != 0u)) {
-                        const uint32_t so = (uint32_t)(rowoff + cj), si = site0 + (uint32_t)cj;
+                        const uint32_t so = (uint32_t)(rowoff + rot + cj), si = site0 + (uint32_t)(rot + cj);
 #pragma unroll
                         for (int w = 0; w < 4; ++w) {
                             const bool pred = nb[w] != 0u;
@@ -544,6 +549,8 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
     if (want < 3) want = 3;
     p->mirror = 0;
     if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = atoi(e) ? 1u : 0u;
+    p->rotate = 1;
+    if (const char* e = getenv("PGG_RING_ROTATE")) p->rotate = atoi(e) ? 1u : 0u;
     const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
                          + (p->mirror ? 3 * p->pitch : 0);
     while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 256) --want;
