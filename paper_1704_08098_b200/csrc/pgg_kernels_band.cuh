@@ -176,11 +176,12 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
     const uint32_t b = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t L = a.L;
-    const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
-    const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
     const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8u * NS;
 
+    // programmatic dependent launch, as in pgg_kernels_ring.cuh: set up while the previous
+    // phase drains, touch the lattice and the phase order only after griddepcontrol.wait
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (int q = threadIdx.x; q < kTableSize; q += kBandThreads)
         tbl[q] = a.tables[(size_t)b * kTableSize + q];
     if (threadIdx.x == 0) {
@@ -192,6 +193,9 @@ phase_band_kernel(PhaseArgs a, uint32_t m, uint32_t k, BandPlan g)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
+    const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
 
     const uint32_t strip = blockIdx.x / g.nb, band = blockIdx.x - strip * g.nb;
     const uint32_t S0 = (uint32_t)(((unsigned long long)band * g.n_super) / g.nb);
@@ -468,11 +472,21 @@ inline int band_plan(int fmt, uint32_t L, uint32_t B, BandPlan* p)
 inline void band_launch(const BandPlan& p, int fmt, const PhaseArgs& a, uint32_t m, uint32_t k,
                         uint32_t B, cudaStream_t stream)
 {
-    dim3 grid(p.n_strips * p.nb, B);
+    static const bool pdl = [] { const char* e = getenv("PGG_PDL"); return e == nullptr || atoi(e) != 0; }();
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.n_strips * p.nb, B);
+    cfg.blockDim = dim3(kBandThreads);
+    cfg.dynamicSmemBytes = p.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
     if (fmt == kFmtU8)
-        phase_band_kernel<kFmtU8><<<grid, kBandThreads, p.smem_bytes, stream>>>(a, m, k, p);
+        cudaLaunchKernelEx(&cfg, phase_band_kernel<kFmtU8>, a, m, k, p);
     else
-        phase_band_kernel<kFmtBits><<<grid, kBandThreads, p.smem_bytes, stream>>>(a, m, k, p);
+        cudaLaunchKernelEx(&cfg, phase_band_kernel<kFmtBits>, a, m, k, p);
 }
 
 }  // namespace pgg
