@@ -318,3 +318,33 @@ def test_config5_full_size(fmt):
     ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 0, 2, n_threads=orc.max_threads())
     assert_same(to_host(d, fmt, L), ref, "C5 lattice after 2 MCS")
     assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
+
+
+@pytest.mark.parametrize("fmt", FMTS)
+def test_oversubscribed_ensemble(fmt):
+    """More CTAs than SMs (300 lattices of L=1024): the streaming kernels are launched with the
+    programmatic-dependent-launch attribute, so a phase may start while CTAs of the previous one are
+    still queued.  Sampled members against the oracle, all members across kernel variants."""
+    B, L, n_mcs = 300, 1024, 4
+    rs = [3.7 + 0.001 * b for b in range(B)]
+    seeds = list(range(100, 100 + B))
+    variants = [v for v in (pgg.VARIANT_V0, pgg.VARIANT_BAND, pgg.VARIANT_RING, pgg.VARIANT_DYN)
+                if pgg.pgg_variant_supported(v, fmt, L)]
+    first = None
+    for v in variants:
+        pgg.pgg_set_variant(v)
+        d = empty_lattice(fmt, L, B)
+        cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+        pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, n_mcs, cnt)
+        torch.cuda.synchronize()
+        if first is None:
+            first = (d, cnt)
+            for b in (0, 149, 299):
+                ref = orc.init(L, 0.5, seeds[b])
+                ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs,
+                                          n_threads=orc.max_threads())
+                assert_same(to_host(d[b], fmt, L), ref, f"member {b}")
+                assert_same(cnt[b].cpu().numpy().astype(np.uint64), ref_counts)
+        else:
+            assert torch.equal(d, first[0]) and torch.equal(cnt, first[1]), f"variant {v} differs from variant {variants[0]}"
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
