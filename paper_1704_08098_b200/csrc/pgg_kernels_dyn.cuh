@@ -296,7 +296,7 @@ inline int dyn_plan_nw(uint32_t L, uint32_t B, RingPlan* p)
         e = cudaFuncSetAttribute(phase_dyn_kernel<NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
         if (e != cudaSuccess) return (int)e;
     }
-    int rc = ring_plan(kFmtU8, L, B, p);
+    int rc = ring_plan(kFmtU8, L, B, p, false);
     if (rc != 0) return rc;
     p->mirror = 0;
     const uint32_t max_chunks = (p->n_super + p->nb - 1) / p->nb + 1;

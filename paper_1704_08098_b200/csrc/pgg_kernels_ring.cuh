@@ -74,6 +74,7 @@ struct RingPlan {
     uint32_t smem_bytes;
     uint32_t mirror;     // 1: three mirror rows in front of slot 0; 0: wrapping stencil reads
     uint32_t rotate;     // 1: column tasks rotate over the warps from step to step
+    uint32_t fullrow;    // 1: the strip is the whole row, no halo columns, one bulk copy per chunk (FR)
 };
 
 // s at offset `off` (site units) from ring0; off may reach into the mirror rows (< 0)
@@ -93,16 +94,27 @@ __device__ __forceinline__ int ring_getw(const uint8_t* ring0, int off, int wrap
 }
 
 // Level 1 (a3, a4): draw, neighbour compare.  Returns true if the site goes on to level 2.
-template <int FMT>
+// Offset of the neighbour y of the site at soff.  FR ("full row": the strip is the whole lattice
+// row, staged without halo columns, rows contiguous in shared memory): a horizontal step stays
+// inside the row, colmask = row length in site units - 1 (a power of two minus one).
+template <bool FR>
+__device__ __forceinline__ int ring_nbr(int soff, uint32_t dir, int e, int colmask)
+{
+    if (!FR) return soff + e;
+    const int m = dir >= 2u ? colmask : -1;
+    return (soff & ~m) | ((soff + e) & m);
+}
+
+template <int FMT, bool FR = false>
 __device__ __forceinline__ bool ring_level1(uint2 e, const uint8_t* ring0, const int* __restrict__ eoff,
-                                            const StepKey& sk, uint4& out, int wrap)
+                                            const StepKey& sk, uint4& out, int wrap, int colmask = 0)
 {
     uint32_t x0, u;
     step_draw(sk, e.y, x0, u);
     const uint32_t dir = x0 >> 30;  // 0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1)
     const int soff = (int)e.x;
     const int sx = ring_get<FMT>(ring0, soff);
-    const int sy = ring_getw<FMT>(ring0, soff + eoff[dir], wrap);  // wrap == 0 with mirror rows
+    const int sy = ring_getw<FMT>(ring0, ring_nbr<FR>(soff, dir, eoff[dir], colmask), wrap);  // wrap == 0 with mirror rows
     out = make_uint4(e.x | (dir << 30) | ((uint32_t)sx << 29), e.y, u, 0u);
     return sx != sy;
 }
@@ -123,15 +135,42 @@ __device__ __forceinline__ int ring_stencil(int soff, uint32_t dir, int sx, cons
          + G(soff + f2) + G(soff - f2) - G(p1 + f2) - G(p1 - f2);
 }
 
-// `wrap_below`: sites with soff below it (ring row 0) take the wrapping stencil; 0 with mirror rows.
+// The stencil of a site near an end of its row in FR mode (and/or in ring row 0): row and column
+// parts of every offset are formed separately, the column part wraps inside the row.
 template <int FMT>
+__device__ __forceinline__ int ring_stencil_fr(int soff, uint32_t dir, int sx, const uint8_t* ring0, int wrap,
+                                               int colmask)
+{
+    const int col = soff & colmask, rowbase = soff - col, ps = colmask + 1;
+    const int er = dir == 0u ? -1 : dir == 1u ? 1 : 0, ec = dir == 2u ? -1 : dir == 3u ? 1 : 0;
+    const int fr = dir < 2u ? 0 : 1, fc = dir < 2u ? 1 : 0;
+    auto S = [&](int a, int b) {
+        int o = rowbase + (a * er + b * fr) * ps + ((col + a * ec + b * fc) & colmask);
+        o += (o >> 31) & wrap;
+        return ring_get<FMT>(ring0, o);
+    };
+    return S(-2, 0) + S(-1, 0) - S(2, 0) - S(3, 0) + 3 * (2 * sx - 1)
+         + 2 * (S(-1, 1) + S(-1, -1) - S(2, 1) - S(2, -1))
+         + S(0, 2) + S(0, -2) - S(1, 2) - S(1, -2);
+}
+
+// `wrap_below`: sites with soff below it (ring row 0) take the wrapping stencil; 0 with mirror rows.
+template <int FMT, bool FR = false>
 __device__ __forceinline__ int ring_accept(int soff, uint32_t dir, int sx, uint32_t site, uint32_t u,
                                            const uint8_t* ring0, const int* __restrict__ eoff,
                                            uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl,
-                                           int wrap, int wrap_below)
+                                           int wrap, int wrap_below, int colmask = 0)
 {
-    const int dA = soff < wrap_below ? ring_stencil<FMT, true>(soff, dir, sx, ring0, eoff, wrap)
-                                     : ring_stencil<FMT, false>(soff, dir, sx, ring0, eoff, 0);
+    int dA;
+    if (FR) {
+        const int col = soff & colmask;
+        dA = (soff < wrap_below || col < 3 || col > colmask - 3)
+                 ? ring_stencil_fr<FMT>(soff, dir, sx, ring0, wrap, colmask)
+                 : ring_stencil<FMT, false>(soff, dir, sx, ring0, eoff, 0);
+    } else {
+        dA = soff < wrap_below ? ring_stencil<FMT, true>(soff, dir, sx, ring0, eoff, wrap)
+                               : ring_stencil<FMT, false>(soff, dir, sx, ring0, eoff, 0);
+    }
     // table_index(dA, ds) = (ds + 1) * 51 + dA + 25 with ds = 2 s_x - 1
     if (u < tbl[sx * 102 + dA + 25]) {
         if (FMT == kFmtU8)
@@ -144,13 +183,13 @@ __device__ __forceinline__ int ring_accept(int soff, uint32_t dir, int sx, uint3
 }
 
 // Level 2 on a Q2 entry (soff | dir << 30 | s_x << 29, site, u)
-template <int FMT>
+template <int FMT, bool FR = false>
 __device__ __forceinline__ int ring_level2(uint4 w, const uint8_t* ring0, const int* __restrict__ eoff,
                                            uint8_t* __restrict__ lat, const uint32_t* __restrict__ tbl,
-                                           int wrap, int wrap_below)
+                                           int wrap, int wrap_below, int colmask = 0)
 {
-    return ring_accept<FMT>((int)(w.x & 0x1FFFFFFFu), w.x >> 30, (int)((w.x >> 29) & 1u), w.y, w.z, ring0, eoff,
-                            lat, tbl, wrap, wrap_below);
+    return ring_accept<FMT, FR>((int)(w.x & 0x1FFFFFFFu), w.x >> 30, (int)((w.x >> 29) & 1u), w.y, w.z, ring0,
+                                eoff, lat, tbl, wrap, wrap_below, colmask);
 }
 
 // Levels 1 and 2 of one queued site without the Q2 entry in between (the inline path)
@@ -159,25 +198,30 @@ struct RingDraw {
     int sx;
     bool go;
 };
-template <int FMT>
+template <int FMT, bool FR = false>
 __device__ __forceinline__ RingDraw ring_draw(uint2 e, const uint8_t* ring0, const int* __restrict__ eoff,
-                                              const StepKey& sk, int wrap)
+                                              const StepKey& sk, int wrap, int colmask = 0)
 {
     RingDraw d;
     uint32_t x0;
     step_draw(sk, e.y, x0, d.u);
     d.dir = x0 >> 30;
     d.sx = ring_get<FMT>(ring0, (int)e.x);
-    d.go = d.sx != ring_getw<FMT>(ring0, (int)e.x + eoff[d.dir], wrap);
+    d.go = d.sx != ring_getw<FMT>(ring0, ring_nbr<FR>((int)e.x, d.dir, eoff[d.dir], colmask), wrap);
     return d;
 }
 
 // FULL: every strip is W bytes wide and every warp has an active row in every step (no ragged
 // edges: the per-lane and per-step guards of the scan drop out).
-template <int FMT, bool FULL>
+// FR ("full row", implies FULL): one strip = the whole lattice row, staged without halo columns,
+// so the rows of a chunk are contiguous in global AND shared memory and arrive as ONE bulk copy
+// (rows of 512 B ... 8 KB copied singly stream at a fraction of the rate, profiles/
+// r1_ring_design_notes.md); the periodic column wrap is resolved in the few sites near a row end.
+template <int FMT, bool FULL, bool FR>
 __global__ void __launch_bounds__(kRingThreads, 1)
 phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
 {
+    constexpr int kHalo = FR ? 0 : kRingHaloB;
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const uint32_t NS = g.NS;
     const int RC = (int)g.RC, pitch = (int)g.pitch;
@@ -231,7 +275,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         const bool left_edge = j0b == 0, right_edge = j0b + wb == rb;
         const uint32_t ring_s = smem_u32(ring0);
         const uint32_t n_chunks = n_steps ? n_steps + 1 : 0;
-        const uint32_t row_tx = (uint32_t)(wb + 2 * kRingHaloB);
+        const uint32_t row_tx = (uint32_t)(wb + 2 * kHalo);
         // first lattice row of chunk kc: the first active row of step S0 + kc - 1 (mod L)
         int row0 = (int)(((long long)RC * ((long long)S0 - 1) + ci) % (long long)L);
         if (row0 < 0) row0 += (int)L;
@@ -243,6 +287,16 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
             const bool mirror = use_mirror && slot == NS - 1;     // its last three rows are also staged above slot 0
             if (lane == 0) mbar_expect_tx(bar, (uint32_t)(RC - r_lo + (mirror ? 3 : 0)) * row_tx);
             __syncwarp();
+            if (FR) {
+                // rows r_lo .. RC-1 of the chunk are contiguous in the lattice unless they cross its end
+                const int g0 = (int)((uint32_t)(row0 + r_lo) % L), n = RC - r_lo;
+                const int n1st = min(n, (int)L - g0);
+                const uint32_t dst = ring_s + (slot * (uint32_t)RC + (uint32_t)r_lo) * (uint32_t)pitch;
+                if (lane == 0) {
+                    bulk_g2s(dst, lat + (size_t)g0 * (size_t)rb, (uint32_t)(n1st * rb), bar);
+                    if (n1st < n) bulk_g2s(dst + (uint32_t)(n1st * rb), lat, (uint32_t)((n - n1st) * rb), bar);
+                }
+            } else
             for (int q = r_lo + lane; q < RC + (mirror ? 3 : 0); q += 32) {
                 const int rr = q < RC ? q : q - 3;  // q >= RC: rows RC-3 .. RC-1 once more
                 const int gi = (int)((uint32_t)(row0 + rr) % L);
@@ -283,6 +337,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         const int ps_sites = (FMT == kFmtU8) ? pitch : 8 * pitch;
         const int wrap = use_mirror ? 0 : ((FMT == kFmtU8) ? ring_bytes : 8 * ring_bytes);
         const int wrap_below = use_mirror ? 0 : ps_sites;
+        const int colmask = FR ? ps_sites - 1 : 0;  // FR: pitch = row length, a power of two
         // Q1 is linear, entries [0, n1); Q2 is a ring of kRingQ2Cap entries, [h2, h2 + n2).
         // o1 / o2 = how many entries at the front were queued by the previous step (they
         // must be finished before this step ends, when their rows are released).
@@ -293,7 +348,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         uint32_t rel_slot = 0;                 // slot of chunk s - 1
         // this lane's 16 bytes of the warp's active row: byte offset from ring0, and the
         // lattice site index of the first of them
-        int rowoff = (int)slot * slot_bytes + 4 * rho * pitch + kRingHaloB + colb;
+        int rowoff = (int)slot * slot_bytes + 4 * rho * pitch + kHalo + colb;
         // byte offset from this lane's 16 bytes to the same columns one lattice row up
         const int up_wrapped = (use_mirror || rho != 0) ? -pitch : ring_bytes - pitch;
         int upoff = (slot == 0) ? up_wrapped : -pitch;
@@ -308,7 +363,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         // level 2 on the first `cnt` (<= 32) entries of Q2
         auto run_level2 = [&](uint32_t cnt) {
             if ((uint32_t)lane < cnt)
-                delta += ring_level2<FMT>(q2[(h2 + lane) & (kRingQ2Cap - 1)], ring0, eoff, lat, tbl, wrap, wrap_below);
+                delta += ring_level2<FMT, FR>(q2[(h2 + lane) & (kRingQ2Cap - 1)], ring0, eoff, lat, tbl, wrap, wrap_below, colmask);
             __syncwarp();  // entries are read before a later append may overwrite them
             h2 += cnt;
             n2 -= cnt;
@@ -317,7 +372,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         // Q2 append of one level-1 batch whose first `n_old` lanes hold old entries
         auto push2 = [&](bool go, const uint4& w, uint32_t n_old) {
             if (!RingCfg<FMT>::q2) {
-                if (go) delta += ring_level2<FMT>(w, ring0, eoff, lat, tbl, wrap, wrap_below);
+                if (go) delta += ring_level2<FMT, FR>(w, ring0, eoff, lat, tbl, wrap, wrap_below, colmask);
                 return;
             }
             const uint32_t mk = __ballot_sync(0xFFFFFFFFu, go);
@@ -335,15 +390,15 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
             if (!RingCfg<FMT>::q2) {
                 if ((uint32_t)lane < cnt) {
                     const uint2 e = q1[head + lane];
-                    const RingDraw d = ring_draw<FMT>(e, ring0, eoff, sk, wrap);
+                    const RingDraw d = ring_draw<FMT, FR>(e, ring0, eoff, sk, wrap, colmask);
                     if (d.go)
-                        delta += ring_accept<FMT>((int)e.x, d.dir, d.sx, e.y, d.u, ring0, eoff, lat, tbl, wrap, wrap_below);
+                        delta += ring_accept<FMT, FR>((int)e.x, d.dir, d.sx, e.y, d.u, ring0, eoff, lat, tbl, wrap, wrap_below, colmask);
                 }
                 return;
             }
             uint4 w;
             bool go = false;
-            if ((uint32_t)lane < cnt) go = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, w, wrap);
+            if ((uint32_t)lane < cnt) go = ring_level1<FMT, FR>(q1[head + lane], ring0, eoff, sk, w, wrap, colmask);
             push2(go, w, n_old);
         };
         // full batches from the front of Q1 (two at a time while 64 wait); the leftover
@@ -355,18 +410,18 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
                 do {
                     if (!RingCfg<FMT>::q2) {  // two independent Philox chains, then the two stencils
                         const uint2 ea = q1[head + lane], eb = q1[head + 32 + lane];
-                        const RingDraw da = ring_draw<FMT>(ea, ring0, eoff, sk, wrap);
-                        const RingDraw db = ring_draw<FMT>(eb, ring0, eoff, sk, wrap);
+                        const RingDraw da = ring_draw<FMT, FR>(ea, ring0, eoff, sk, wrap, colmask);
+                        const RingDraw db = ring_draw<FMT, FR>(eb, ring0, eoff, sk, wrap, colmask);
                         if (da.go)
-                            delta += ring_accept<FMT>((int)ea.x, da.dir, da.sx, ea.y, da.u, ring0, eoff, lat, tbl, wrap, wrap_below);
+                            delta += ring_accept<FMT, FR>((int)ea.x, da.dir, da.sx, ea.y, da.u, ring0, eoff, lat, tbl, wrap, wrap_below, colmask);
                         if (db.go)
-                            delta += ring_accept<FMT>((int)eb.x, db.dir, db.sx, eb.y, db.u, ring0, eoff, lat, tbl, wrap, wrap_below);
+                            delta += ring_accept<FMT, FR>((int)eb.x, db.dir, db.sx, eb.y, db.u, ring0, eoff, lat, tbl, wrap, wrap_below, colmask);
                         head += 64u;
                         continue;
                     }
                     uint4 wa, wb2;
-                    const bool ga = ring_level1<FMT>(q1[head + lane], ring0, eoff, sk, wa, wrap);
-                    const bool gb = ring_level1<FMT>(q1[head + 32 + lane], ring0, eoff, sk, wb2, wrap);
+                    const bool ga = ring_level1<FMT, FR>(q1[head + lane], ring0, eoff, sk, wa, wrap, colmask);
+                    const bool gb = ring_level1<FMT, FR>(q1[head + 32 + lane], ring0, eoff, sk, wb2, wrap, colmask);
                     push2(ga, wa, head ? 0u : o1);
                     push2(gb, wb2, 0u);
                     head += 64u;
@@ -403,8 +458,9 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
                     wc = *reinterpret_cast<const uint4*>(rowp);
                     wu = *reinterpret_cast<const uint4*>(rowp + upoff);
                     wd = *reinterpret_cast<const uint4*>(rowp + pitch);
-                    pv = *reinterpret_cast<const uint32_t*>(rowp - 4);
-                    nx = *reinterpret_cast<const uint32_t*>(rowp + 16);
+                    // FR: the word left of the row's first / right of its last is the row's other end
+                    pv = *reinterpret_cast<const uint32_t*>(rowp - 4 + ((FR && colb + rot == 0) ? pitch : 0));
+                    nx = *reinterpret_cast<const uint32_t*>(rowp + 16 - ((FR && colb + rot + 16 == pitch) ? pitch : 0));
                 }
                 const uint32_t c4[4] = {wc.x, wc.y, wc.z, wc.w};
                 const uint32_t u4[4] = {wu.x, wu.y, wu.z, wu.w};
@@ -502,7 +558,7 @@ inline bool ring_supported(int fmt, uint32_t L)
     return fmt == kFmtU8 ? (L % 16 == 0) : (L % 128 == 0);  // rows are multiples of 16 bytes
 }
 
-inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
+inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p, bool allow_fullrow = true)
 {
     static int sm_count = 0, smem_optin = 0;
     if (sm_count == 0) {
@@ -513,14 +569,14 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
         if (e != cudaSuccess) return (int)e;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtU8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(phase_ring_kernel<kFmtBits, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
-        if (e != cudaSuccess) return (int)e;
+        const void* kernels[6] = {
+            (const void*)phase_ring_kernel<kFmtU8, false, false>, (const void*)phase_ring_kernel<kFmtU8, true, false>,
+            (const void*)phase_ring_kernel<kFmtU8, true, true>, (const void*)phase_ring_kernel<kFmtBits, false, false>,
+            (const void*)phase_ring_kernel<kFmtBits, true, false>, (const void*)phase_ring_kernel<kFmtBits, true, true>};
+        for (const void* kern : kernels) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+            if (e != cudaSuccess) return (int)e;
+        }
         sm_count = sms;
     }
     p->row_bytes = fmt == kFmtU8 ? L : L / 8;
@@ -535,7 +591,9 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
     p->n_strips = (p->row_bytes + p->W - 1) / p->W;
     p->R = kRingConsumers >> tpr_log2;
     p->RC = 4 * p->R;
-    p->pitch = p->W + 2 * kRingHaloB;
+    p->fullrow = (allow_fullrow && p->n_strips == 1 && p->W == p->row_bytes) ? 1u : 0u;
+    if (const char* e = getenv("PGG_RING_FULLROW")) p->fullrow = (p->fullrow && atoi(e)) ? 1u : 0u;
+    p->pitch = p->fullrow ? p->W : p->W + 2 * kRingHaloB;
     p->slot_bytes = p->RC * p->pitch;
     p->n_groups = L / 4;
     p->n_super = (p->n_groups + p->R - 1) / p->R;
@@ -548,7 +606,7 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p)
     if (want > (uint32_t)kRingMaxSlots) want = kRingMaxSlots;
     if (want < 3) want = 3;
     p->mirror = 0;
-    if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = atoi(e) ? 1u : 0u;
+    if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = (atoi(e) && !p->fullrow) ? 1u : 0u;
     p->rotate = 1;
     if (const char* e = getenv("PGG_RING_ROTATE")) p->rotate = atoi(e) ? 1u : 0u;
     const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
@@ -576,11 +634,13 @@ inline void ring_launch(const RingPlan& p, int fmt, const PhaseArgs& a, uint32_t
     cfg.numAttrs = 1;
     const bool full = p.row_bytes % p.W == 0 && p.n_groups % p.R == 0;
     if (fmt == kFmtU8) {
-        if (full) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, true>, a, m, k, p);
-        else cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, false>, a, m, k, p);
+        if (p.fullrow) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, true, true>, a, m, k, p);
+        else if (full) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, true, false>, a, m, k, p);
+        else cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtU8, false, false>, a, m, k, p);
     } else {
-        if (full) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, true>, a, m, k, p);
-        else cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, false>, a, m, k, p);
+        if (p.fullrow) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, true, true>, a, m, k, p);
+        else if (full) cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, true, false>, a, m, k, p);
+        else cudaLaunchKernelEx(&cfg, phase_ring_kernel<kFmtBits, false, false>, a, m, k, p);
     }
 }
 

@@ -321,7 +321,7 @@ inline int split_plan(uint32_t L, uint32_t B, RingPlan* p)
         e = cudaFuncSetAttribute(phase_split_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
         if (e != cudaSuccess) return (int)e;
     }
-    int rc = ring_plan(kFmtU8, L, B, p);
+    int rc = ring_plan(kFmtU8, L, B, p, false);
     if (rc != 0) return rc;
     p->mirror = 0;
     const uint32_t max_chunks = (p->n_super + p->nb - 1) / p->nb + 1;
