@@ -348,3 +348,18 @@ def test_oversubscribed_ensemble(fmt):
         else:
             assert torch.equal(d, first[0]) and torch.equal(cnt, first[1]), f"variant {v} differs from variant {variants[0]}"
     pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+
+
+@pytest.mark.parametrize("L", [4096, 8192])
+def test_fullrow_strip_sizes(L):
+    """uint8 lattices whose row is one strip (512 B ... 8 KB): staged without halo columns, one bulk copy
+    per chunk, column wrap resolved in the sites near a row end (RING full-row mode)."""
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    seed, r, n_mcs = 40 + L, 3.8, 2
+    lat0 = orc.init(L, 0.5, seed)
+    ref = lat0.copy()
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 5, n_mcs, n_threads=orc.max_threads())
+    got, counts = gpu_sweep(lat0, pgg.FMT_U8, r, seed, pgg.ORDER_IID, 5, n_mcs)
+    assert pgg.pgg_get_variant_used() == pgg.VARIANT_RING
+    assert_same(got, ref, f"lattice L={L}")
+    assert_same(counts, ref_counts, f"counts L={L}")
