@@ -363,3 +363,20 @@ def test_fullrow_strip_sizes(L):
     assert pgg.pgg_get_variant_used() == pgg.VARIANT_RING
     assert_same(got, ref, f"lattice L={L}")
     assert_same(counts, ref_counts, f"counts L={L}")
+
+
+def test_large_lattice_L32768():
+    """A 1 GiB uint8 lattice (4 strips of 8 KB, site indices up to 2^30): one MCS against the oracle."""
+    L, seed, r = 32768, 9, 3.8
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    d = empty_lattice(pgg.FMT_U8, L)
+    pgg.pgg_init_lattice(d, pgg.FMT_U8, L, 0.5, seed)
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    pgg.pgg_sweep(d, pgg.FMT_U8, L, r, K, seed, pgg.ORDER_IID, 7, 1, cnt)
+    torch.cuda.synchronize()
+    ref = orc.init(L, 0.5, seed)
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 7, 1, n_threads=orc.max_threads())
+    got = d.cpu().numpy()
+    del d
+    assert np.array_equal(got, ref), "L=32768 lattice differs"
+    assert int(cnt.item()) == int(ref_counts[0])
