@@ -24,10 +24,20 @@
 //     A_x - A_y are ring0[soff + a e + b f] with six row bases shared between
 //     them;
 //   * level 1 runs two batches of 32 queued sites at once when 64 are waiting,
-//     so two independent Philox chains hide each other's multiply latency.
+//     so two independent Philox chains hide each other's multiply latency;
+//   * uint8 runs the stencil inline on the lanes whose drawn neighbour differs
+//     (a second queue fills its batches only half: a site may wait one step
+//     only); the bit-packed instantiation keeps Q2;
+//   * launches carry the programmatic-dependent-launch attribute: a CTA sets up
+//     while the previous phase drains and executes griddepcontrol.wait before it
+//     touches the lattice;
+//   * the 16 column tasks of a step rotate over the warps, so that no warp is
+//     tied to the busiest columns of the band;
+//   * full-row mode (FR): when the strip is the whole lattice row the halo
+//     columns are dropped and a chunk arrives as ONE bulk copy.
 //
-// Geometry, producer, barriers and the two-level compaction (scan -> Q1 ->
-// Philox -> Q2 -> stencil) are those of pgg_kernels_band.cuh:
+// Geometry, producer, barriers and the compaction (scan -> Q1 -> Philox
+// [-> Q2] -> stencil) are those of pgg_kernels_band.cuh:
 //
 //   strip  = W = tpr * 512 bytes of every lattice row (+ 16-byte halo each side)
 //   band   = the consecutive lattice rows of a strip one persistent CTA streams
