@@ -21,6 +21,7 @@ _LIB = _HERE / "liboracle_pgg.so"
 
 ORDER_IID = 0
 ORDER_PERM = 1
+ORDER_DTILE = 2  # the paper's double-tiling schedule
 
 
 def build(force: bool = False) -> Path:
@@ -75,6 +76,14 @@ def lib() -> C.CDLL:
         L.orc_phase.argtypes = [u8p, C.c_int, u32p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32,
                                 C.c_int, u32p, C.c_int]
         L.orc_phase.restype = C.c_int64
+        L.orc_dtile_type.argtypes = [C.c_int, C.c_int]
+        L.orc_dtile_type.restype = C.c_int
+        L.orc_dtile_draw.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32,
+                                     C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), u32p]
+        L.orc_dtile_draw.restype = None
+        L.orc_dtile_part.argtypes = [u8p, C.c_int, u32p, C.c_uint64, C.c_uint32, C.c_int, C.c_int,
+                                     C.c_int]
+        L.orc_dtile_part.restype = C.c_int64
         L.orc_sweep.argtypes = [u8p, C.c_int, C.c_double, C.c_double, C.c_uint64, C.c_int,
                                 C.c_uint32, C.c_uint32, u64p, C.c_uint32, u8p, C.c_int]
         L.orc_sweep.restype = C.c_int
@@ -202,6 +211,26 @@ def phase(lat, table, seed, t, k, c, visit=0, perm=None, n_threads=1) -> int:
         p = _u32(perm)
     return int(lib().orc_phase(_u8(lat), lat.shape[0], _u32(table), seed, t, k, c, visit, p,
                                n_threads))
+
+
+def dtile_type(I, J) -> int:
+    return int(lib().orc_dtile_type(I, J))
+
+
+def dtile_draw(seed, d, t, p):
+    """(domain row, domain column, direction, u) of pick p of domain d in MCS t."""
+    a, b, di = C.c_int(0), C.c_int(0), C.c_int(0)
+    u = np.zeros(1, dtype=np.uint32)
+    lib().orc_dtile_draw(seed, d, t, p, C.byref(a), C.byref(b), C.byref(di), _u32(u))
+    return a.value, b.value, di.value, int(u[0])
+
+
+def dtile_part(lat, table, seed, t, q, visit=0, n_threads=1) -> int:
+    """In-place part q (domains of type q) of MCS t of the double-tiling schedule; count delta."""
+    assert lat.dtype == np.uint8 and lat.flags.c_contiguous and lat.shape[0] % 8 == 0
+    table = np.ascontiguousarray(table, dtype=np.uint32)
+    return int(lib().orc_dtile_part(_u8(lat), lat.shape[0], _u32(table), seed, t, q, visit,
+                                    n_threads))
 
 
 def sweep(lat, r, K, seed, order_mode=ORDER_IID, t_begin=0, n_mcs=1, snap_every=0, n_threads=1):

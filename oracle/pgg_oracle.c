@@ -38,9 +38,11 @@
 #define ORC_TAG_ORDER 2u
 #define ORC_TAG_STEP 3u
 #define ORC_TAG_RS 4u
+#define ORC_TAG_DTILE 5u /* T2: the paper's double-tiling schedule */
 
 #define ORC_ORDER_IID 0  /* D5 */
 #define ORC_ORDER_PERM 1
+#define ORC_ORDER_DTILE 2 /* PAPER.md:75-93, readings T1-T4 */
 
 /* ------------------------------------------------------------------------- */
 /* D1. Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).  The paper only says */
@@ -347,8 +349,97 @@ int64_t orc_phase(uint8_t *lat, int L, const uint32_t table[153], uint64_t seed,
 }
 
 /* ------------------------------------------------------------------------- */
+/* The paper's own parallel schedule: double tiling decomposition              */
+/* (Fig. 2, Fig. 3).  The lattice is cut into 4x4 domains      */
+/* ("domain size S to be 4x4"); domain (I,J) = (i>>2, j>>2) has    */
+/* type 2*(I&1) + (J&1) in {0,1,2,3} -- the paper's types 1,2,3,4, laid out    */
+/* "linearly in sequences of 2 (1,2,1,2,... or 3,4,3,4,...)", so */
+/* L % 8 == 0.  A full MCS is four parts, the types "updated  */
+/* in turn" 1,2,3,4; in a part every domain of that type is      */
+/* updated by "independent parallel random sequential updating". */
+/* Readings where the paper is silent (S15, T1-T4):       */
+/*  T1 picks per domain per part = 16 = the domain's sites, so that one MCS is */
+/*     4 parts x L^2/64 domains x 16 = L^2 elementary steps;     */
+/*  T2 pick p of domain d = I*(L/4)+J in MCS t draws (x0,x1,x2,.) =            */
+/*     Philox(ctr = (d, t, p, DTILE)); focal site = domain row x0>>30, domain  */
+/*     column (x0>>28)&3; neighbour direction = x2>>30 (as D6); u = x1;        */
+/*  T3 domain origins are fixed (no shift between MCS);                        */
+/*  T4 the picks of one domain are sequential: pick p sees picks 0..p-1.       */
+/* Race freedom: a step reads within Manhattan distance 3 of x (S1) and writes */
+/* x; two domains of one type are separated by a 4-site gap in each axis, so   */
+/* no read of one reaches into the other ("three lines outward").  */
+/* ------------------------------------------------------------------------- */
+int orc_dtile_type(int I, int J)
+{
+    return 2 * (I & 1) + (J & 1);
+}
+
+void orc_dtile_draw(uint64_t seed, uint32_t d, uint32_t t, uint32_t p, int *a, int *b, int *dir,
+                    uint32_t *u)
+{
+    uint32_t key[2];
+    seed_key(seed, key);
+    uint32_t ctr[4] = {d, t, p, ORC_TAG_DTILE};
+    uint32_t x[4];
+    orc_philox4x32_10(ctr, key, x);
+    *a = (int)(x[0] >> 30);
+    *b = (int)((x[0] >> 28) & 3u);
+    *dir = (int)(x[2] >> 30);
+    *u = x[1];
+}
+
+/* The 16 sequential elementary steps of domain (I,J) in MCS t (T1, T4).       */
+static int64_t dtile_domain(uint8_t *lat, int L, const uint32_t table[153], uint64_t seed,
+                            uint32_t t, int I, int J)
+{
+    int64_t delta = 0;
+    uint32_t d = (uint32_t)(I * (L / 4) + J);
+    for (uint32_t p = 0; p < 16; ++p) {
+        int a, b, dir;
+        uint32_t u;
+        orc_dtile_draw(seed, d, t, p, &a, &b, &dir, &u);
+        int i = 4 * I + a, j = 4 * J + b;
+        size_t site = (size_t)i * (size_t)L + (size_t)j;
+        int old = lat[site];
+        int neu = orc_step_given_draw(lat, L, table, i, j, dir, u);
+        lat[site] = (uint8_t)neu;
+        delta += neu - old;
+    }
+    return delta;
+}
+
+/* Part q of MCS t: every domain of type q.  visit: 0 raster over the domains, */
+/* 1 reverse raster -- the result must not depend on it.  n_threads > 1 splits */
+/* the domain rows over OpenMP threads (same result, by the race freedom       */
+/* above).  Returns the signed change of the cooperator count.                 */
+int64_t orc_dtile_part(uint8_t *lat, int L, const uint32_t table[153], uint64_t seed, uint32_t t,
+                       int q, int visit, int n_threads)
+{
+    int M = L / 4;
+    int64_t delta = 0;
+    if (n_threads <= 1 || visit != 0) {
+        for (int n = 0; n < M * M; ++n) {
+            int m = visit == 1 ? M * M - 1 - n : n;
+            int I = m / M, J = m % M;
+            if (orc_dtile_type(I, J) == q)
+                delta += dtile_domain(lat, L, table, seed, t, I, J);
+        }
+    } else {
+#ifdef _OPENMP
+#pragma omp parallel for num_threads(n_threads) reduction(+ : delta) schedule(static)
+#endif
+        for (int I = 0; I < M; ++I)
+            for (int J = 0; J < M; ++J)
+                if (orc_dtile_type(I, J) == q)
+                    delta += dtile_domain(lat, L, table, seed, t, I, J);
+    }
+    return delta;
+}
+
+/* ------------------------------------------------------------------------- */
 /* D6+D7. n_mcs full Monte Carlo steps t = t_begin .. t_begin+n_mcs-1, each 16 */
-/* phases (1 MCS = L^2 elementary steps: 16 phases x L^2/16).     */
+/* phases (1 MCS = L^2 elementary steps: 16 phases x L^2/16), or  */
+/* with order_mode == ORC_ORDER_DTILE the four parts of the paper's schedule.  */
 /* counts[m] = number of cooperators after MCS t_begin+m completes (may be     */
 /* NULL).  If snap_every > 0, the lattice is copied to snaps after every MCS   */
 /* whose 1-based index within this call is a multiple of snap_every.           */
@@ -360,6 +451,8 @@ int orc_sweep(uint8_t *lat, int L, double r, double K, uint64_t seed, int order_
 {
     if (L < 4 || L % 4 != 0 || !(K > 0.0))
         return -1;
+    if (order_mode == ORC_ORDER_DTILE && L % 8 != 0)
+        return -1; /* PAPER.md:93 */
     uint32_t table[153];
     orc_accept_table(r, K, table);
     size_t n = (size_t)L * (size_t)L;
@@ -367,10 +460,15 @@ int orc_sweep(uint8_t *lat, int L, double r, double K, uint64_t seed, int order_
     size_t n_snap = 0;
     for (uint32_t m = 0; m < n_mcs; ++m) {
         uint32_t t = t_begin + m;
-        uint8_t cls[16];
-        orc_phase_classes(seed, t, order_mode, cls);
-        for (uint32_t k = 0; k < 16; ++k)
-            count += orc_phase(lat, L, table, seed, t, k, cls[k], 0, NULL, n_threads);
+        if (order_mode == ORC_ORDER_DTILE) {
+            for (int q = 0; q < 4; ++q) /* types 1,2,3,4 in turn */
+                count += orc_dtile_part(lat, L, table, seed, t, q, 0, n_threads);
+        } else {
+            uint8_t cls[16];
+            orc_phase_classes(seed, t, order_mode, cls);
+            for (uint32_t k = 0; k < 16; ++k)
+                count += orc_phase(lat, L, table, seed, t, k, cls[k], 0, NULL, n_threads);
+        }
         if (counts)
             counts[m] = (uint64_t)count;
         if (snap_every > 0 && (m + 1) % snap_every == 0) {
