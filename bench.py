@@ -85,6 +85,9 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+ORC_ORDER = 0  # oracle order mode of the cpu_baseline / reference legs (set from --order)
+
+
 def oracle_sample(L: int, max_mcs: int, min_seconds: float):
     """Time the oracle (as it stands) on `max_mcs` MCS of the workload, all host threads."""
     import numpy as np
@@ -93,7 +96,7 @@ def oracle_sample(L: int, max_mcs: int, min_seconds: float):
     lat = orc.init(L, RHO0, SEED)
     done, t0 = 0, time.perf_counter()
     while done < max_mcs:
-        orc.sweep(lat, R, K_NOISE, SEED, orc.ORDER_IID, done, 1, n_threads=threads)
+        orc.sweep(lat, R, K_NOISE, SEED, ORC_ORDER, done, 1, n_threads=threads)
         done += 1
         if time.perf_counter() - t0 >= min_seconds:
             break
@@ -127,10 +130,10 @@ def run_reference(args):
     lat = orc.init(L, RHO0, SEED)
     t = 0
     for _ in range(args.warmup):
-        orc.sweep(lat, R, K_NOISE, SEED, orc.ORDER_IID, t, 1, n_threads=threads); t += 1
+        orc.sweep(lat, R, K_NOISE, SEED, ORC_ORDER, t, 1, n_threads=threads); t += 1
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        orc.sweep(lat, R, K_NOISE, SEED, orc.ORDER_IID, t, 1, n_threads=threads); t += 1
+        orc.sweep(lat, R, K_NOISE, SEED, ORC_ORDER, t, 1, n_threads=threads); t += 1
     dt = time.perf_counter() - t0
     value = args.steps * L * L / dt
     sample = (f"each step = 1 MCS (MCS {args.warmup}..{t - 1}) of the L={L} workload from the "
@@ -168,6 +171,8 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     L, n_mcs = args.L, args.mcs
+    ORDER = {"iid": pgg.ORDER_IID, "perm": pgg.ORDER_PERM, "dtile": pgg.ORDER_DTILE}[args.order]
+    dtile = args.order == "dtile"
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
                "fused": pgg.VARIANT_FUSED, "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND,
@@ -194,15 +199,15 @@ def run_ours(args):
         if args.profile_mcs >= 0:
             # for `ncu --profile-from-start off`: only MCS `profile_mcs` lies in the profiled range
             pm = min(args.profile_mcs, n_mcs - 1)
-            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, pm, None, stream)
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, 0, pm, None, stream)
             torch.cuda.synchronize()
             torch.cuda.profiler.start()
-            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, pm, 1, None, stream)
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, pm, 1, None, stream)
             torch.cuda.synchronize()
             torch.cuda.profiler.stop()
-            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, pm + 1, n_mcs - pm - 1, None, stream)
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, pm + 1, n_mcs - pm - 1, None, stream)
             pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
-        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, n_mcs, d_counts, stream)
+        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, 0, n_mcs, d_counts, stream)
         if i is not None:
             ev_c[i].record(stream)
 
@@ -236,7 +241,7 @@ def run_ours(args):
 
     def e2e_step():
         d_lat.copy_(h_lat0, non_blocking=True)
-        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, pgg.ORDER_IID, 0, n_mcs, d_counts, stream)
+        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, 0, n_mcs, d_counts, stream)
         h_out.copy_(d_lat, non_blocking=True)
         h_counts.copy_(d_counts, non_blocking=True)
         stream.synchronize()
@@ -264,22 +269,27 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (the phase kernel; 16 launches per MCS)
     peak, peak_src = load_peaks()
-    n_phase = 16 * n_mcs * args.steps
+    # (the paper's double-tiling schedule, --order dtile: 4 parts per MCS, each reads N and writes N/4)
+    per_mcs = 4 if dtile else 16
+    n_phase = per_mcs * n_mcs * args.steps
     phase_us = sweep_ms * 1e3 / n_phase            # includes the per-call order/density/finalize kernels
     b_site = 1.0 if fmt == pgg.FMT_U8 else 0.125
-    bytes_per_launch = (L * L + L * L / 16.0) * b_site   # read the lattice, write the active class
+    bytes_per_launch = (L * L + L * L / float(per_mcs)) * b_site   # read the lattice, write the active class
     achieved = bytes_per_launch / (phase_us * 1e-6) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "kernel": "phase kernel (variant %d)" % pgg.pgg_get_variant_used(),
+                "kernel": ("dtile_part_kernel" if dtile else "phase kernel") + " (variant %d)" % pgg.pgg_get_variant_used(),
                 "avg_launch_us": phase_us, "algorithmic_bytes_per_launch": bytes_per_launch,
-                "note": "17 B/update contract bytes (16 phases x (read N + write N/16)), SURVEY 8(d)"
+                "note": ("5 B/update (4 parts x (read N + write N/4)); 16 full Philox draws per domain make this "
+                         "schedule ALU-bound, the HBM fraction is context" if dtile else
+                         "17 B/update contract bytes (16 phases x (read N + write N/16)), SURVEY 8(d)")
                         + ("; the 32 MiB packed lattice is L2-resident, so this is not a DRAM fraction"
                            if fmt == pgg.FMT_BITS else "")}
     tr = ROOT / "profiles" / "traffic.json"
     if tr.exists():
         try:
-            roofline["traffic"] = json.loads(tr.read_text()).get(f"{args.fmt}_L{L}_bytes_per_launch")
+            roofline["traffic"] = json.loads(tr.read_text()).get(
+                f"{args.fmt}_L{L}_bytes_per_launch" + ("_dtile" if dtile else ""))
         except (ValueError, OSError):
             pass
 
@@ -290,7 +300,7 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": f"C5 throughput: single L={L} lattice, Bernoulli(0.5) init seed 1, r={R}, "
                                f"K={K_NOISE}, {n_mcs} MCS per step (init + sweep + fused rho_C trace)",
-                   "fmt": args.fmt, "L": L, "mcs_per_step": n_mcs, "order_mode": "iid",
+                   "fmt": args.fmt, "L": L, "mcs_per_step": n_mcs, "order_mode": args.order,
                    "variant": pgg.pgg_get_variant_used(),
                    "l2": ("inputs larger than L2 (256 MiB lattice re-read every phase)" if lat_bytes > 130e6
                           else "lattice fits L2 by nature of the workload; no flush"),
@@ -326,6 +336,10 @@ def main():
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
     ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band", "ring", "split", "dyn", "resident"])
+    ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"],
+                    help="schedule: the 16-sublattice schedule with i.i.d. (bench default) or permuted classes, or "
+                         "the paper's own double-tiling schedule (PAPER.md:75-93); anything but iid is not the bench workload")
+    ap.add_argument("--r", type=float, default=R, help="synergy factor; anything but 3.8 is not the bench workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-mcs", type=int, default=-1,
                     help="profiling aid: bracket this MCS with cudaProfilerStart/Stop (ncu --profile-from-start off); "
@@ -335,6 +349,8 @@ def main():
                          "pure streaming rate of the phase kernel.  Anything but 0.5 is not the bench workload")
     args = ap.parse_args()
     globals()["RHO0"] = args.rho0
+    globals()["R"] = args.r
+    globals()["ORC_ORDER"] = {"iid": 0, "perm": 1, "dtile": 2}[args.order]
     if args.impl == "reference":
         run_reference(args)
     else:

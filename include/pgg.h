@@ -60,8 +60,18 @@ enum { PGG_FMT_U8 = 0, PGG_FMT_BITS = 1 };
 /* How the 16 phase classes of an MCS are drawn.
  * PGG_ORDER_IID : class of phase k = top 4 bits of word k (default; reproduces
  *                 random-sequential statistics).
- * PGG_ORDER_PERM: a permutation -- classes sorted by (word[c], c).               */
-enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1 };
+ * PGG_ORDER_PERM: a permutation -- classes sorted by (word[c], c).
+ * PGG_ORDER_DTILE: not a class order but the paper's own schedule, the double
+ *   tiling decomposition (Fig. 2): 4x4 domains, domain (I,J) =
+ *   (i>>2, j>>2) of type 2*(I&1) + (J&1), L % 8 == 0; one MCS =
+ *   four parts, types 0,1,2,3 in turn; in a part every domain of
+ *   the type makes 16 sequential elementary steps on its own sites (so that an
+ *   MCS is L^2 steps); pick p of domain d = I*(L/4) + J in MCS t
+ *   draws (x0,x1,x2,.) = Philox4x32-10(ctr = (d, t, p, 5), key = seed): focal
+ *   site = domain row x0>>30, domain column (x0>>28)&3, neighbour direction
+ *   x2>>30 (0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1)), u = x1; x adopts s_y iff
+ *   s_x != s_y and u < T[...] as in every mode.  Kernel variants do not apply. */
+enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
 
 /* Kernel variants of the phase step (all bit-identical).
  * PGG_VARIANT_AUTO picks the fastest one that supports (fmt, L): RESIDENT for
@@ -76,8 +86,10 @@ enum {
     PGG_VARIANT_RING = 6, /* BAND's data movement, consumer cut to the fewest instr.  */
     PGG_VARIANT_SPLIT = 7,/* RING with scanner and worker warps (uint8 only)          */
     PGG_VARIANT_DYN = 8,  /* RING with dynamically assigned tasks, 24 warps (uint8)   */
-    PGG_VARIANT_RESIDENT = 9 /* L <= 512: one CTA per lattice, lattice resident in smem,
+    PGG_VARIANT_RESIDENT = 9,/* L <= 512: one CTA per lattice, lattice resident in smem,
                                 every phase of the call in one launch                  */
+    PGG_VARIANT_DTILE = 10   /* reported by pgg_get_variant_used() after a PGG_ORDER_DTILE
+                                sweep (one thread per 4x4 domain); not selectable       */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:
@@ -105,7 +117,8 @@ int32_t pgg_init_lattice(void* d_lat, int32_t fmt, uint32_t L, double rho0, uint
  * (a, b+c) bit for bit.
  * Errors: PGG_ERR_NULL (d_lat), PGG_ERR_BAD_L, PGG_ERR_ALIGN, PGG_ERR_BAD_PARAM
  * (r, K not finite, K <= 0, t_begin + n_mcs > 2^32), PGG_ERR_UNSUPPORTED
- * (fmt, order_mode), PGG_ERR_CUDA.  n_mcs == 0 is a no-op.                        */
+ * (fmt, order_mode), PGG_ERR_CUDA.  n_mcs == 0 is a no-op.  PGG_ORDER_DTILE needs
+ * L % 8 == 0, else PGG_ERR_BAD_L.                                   */
 int32_t pgg_sweep(void* d_lat, int32_t fmt, uint32_t L, double r, double K, uint64_t seed,
                   int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
                   void* stream);

@@ -22,6 +22,7 @@
 #include "pgg_kernels_split.cuh"
 #include "pgg_kernels_dyn.cuh"
 #include "pgg_kernels_resident.cuh"
+#include "pgg_kernels_dtile.cuh"
 
 namespace {
 
@@ -133,8 +134,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
                    const uint64_t* h_seeds, int32_t order_mode, double rho0, uint32_t t_begin,
                    uint32_t n_mcs, uint64_t* d_counts, cudaStream_t stream)
 {
-    if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM)
+    if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM && order_mode != PGG_ORDER_DTILE)
         return fail(PGG_ERR_UNSUPPORTED, "unknown order_mode %d", order_mode);
+    if (order_mode == PGG_ORDER_DTILE && L % 8 != 0)
+        return fail(PGG_ERR_BAD_L, "L = %u: the double tiling schedule needs L %% 8 == 0 (PAPER.md:93)", L);
     if (!(K > 0.0) || !std::isfinite(K)) return fail(PGG_ERR_BAD_PARAM, "K must be finite and > 0");
     for (uint32_t b = 0; b < B; ++b)
         if (!std::isfinite(h_r[b])) return fail(PGG_ERR_BAD_PARAM, "r[%u] is not finite", b);
@@ -142,7 +145,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         return fail(PGG_ERR_BAD_PARAM, "t_begin + n_mcs exceeds 2^32");
     if (L == 65536) return fail(PGG_ERR_BAD_L, "L = 65536: site index does not fit uint32 counters");
 
-    int variant = g_variant.load();
+    int variant = order_mode == PGG_ORDER_DTILE ? PGG_VARIANT_DTILE : g_variant.load();
     const bool tile_ok = pgg::tile_supported(fmt, L);
     const bool band_ok = pgg::band_supported(fmt, L);
     const bool ring_ok = pgg::ring_supported(fmt, L);
@@ -196,6 +199,28 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     }
 
     const uint32_t chunk = std::min<uint32_t>(n_mcs, 4096u);
+    if (variant == PGG_VARIANT_DTILE) {  // the paper's schedule: four parts per MCS, no class order
+        pgg::PhaseArgs a{};
+        a.lats = d_lats;
+        a.lat_bytes = lattice_bytes(fmt, L);
+        a.seeds = d_seeds;
+        a.tables = d_tables;
+        a.deltas = reinterpret_cast<unsigned long long*>(d_counts);
+        a.L = L;
+        a.n_mcs = n_mcs;
+        a.t_begin = t_begin;
+        for (uint32_t m = 0; m < n_mcs; ++m)
+            for (uint32_t q = 0; q < 4; ++q) {
+                pgg::dtile_launch(fmt, a, m, q, B, stream);
+                PGG_LAUNCHED();
+            }
+        if (d_counts != nullptr) {
+            pgg::finalize_counts_kernel<<<B, 1024, 0, stream>>>(
+                reinterpret_cast<unsigned long long*>(d_counts), n_mcs, d_count0);
+            PGG_LAUNCHED();
+        }
+        return PGG_OK;
+    }
     uint8_t* d_order = nullptr;
     PGG_CUDA(tmp.alloc((void**)&d_order, (size_t)B * chunk * 16));
 
