@@ -3,6 +3,7 @@
     python -m paper_1704_08098_b200.physics stationary [--L 400] [--mcs 20000] [--seeds 101 102 103 104]
                                                        [--order iid|perm] [--rs 3.6 3.65 ...]
     python -m paper_1704_08098_b200.physics decay --r 3.7443 [--L 2048] [--mcs 100000] [--seeds 1..16]
+    python -m paper_1704_08098_b200.physics fig5 [--order dtile|iid] [--mcs 2000]
 
 ``stationary``: rho_C(r) of BASELINE.json configs[1] -- the time average of Eq. (4) over
 the second half of the run, with the standard error from 10 batch means, per (r, seed) and pooled.
@@ -10,6 +11,9 @@ the second half of the run, with the standard error from 10 batch means, per (r,
 delta_eff(t) = -ln[rho(t)/rho(t/8)] / ln 8 (directed percolation: delta = 0.4505; PAPER.md:97,111 place
 the transition in that class).  Every number comes from the integer count traces the kernels produce;
 the arithmetic here is averaging only.
+``fig5``: the timing experiment of the paper's Fig. 5: L = 32 ... 4096 at K = 0.5,
+r = 3.98, wall time per 10^6 full MCS, extrapolated from --mcs MCS timed with CUDA events after a
+warm-up of the same length (the paper ran 10^6 MCS; its GTX 1080 / Xeon times are context only).
 """
 from __future__ import annotations
 
@@ -19,7 +23,7 @@ import math
 
 import numpy as np
 
-from . import (FMT_U8, ORDER_IID, ORDER_PERM, pgg_run_ensemble)
+from . import (FMT_U8, ORDER_DTILE, ORDER_IID, ORDER_PERM, pgg_init_lattice, pgg_run_ensemble, pgg_sweep)
 
 
 def run_traces(L, rs, seeds, K, rho0, n_mcs, order=ORDER_IID, fmt=FMT_U8, chunk=None):
@@ -89,18 +93,42 @@ def decay(r, seeds, L=2048, n_mcs=100000, K=0.5, rho0=0.5, order=ORDER_IID):
     return rows
 
 
+def fig5(order=ORDER_DTILE, n_mcs=2000, Ls=(32, 64, 128, 256, 512, 1024, 2048, 4096), r=3.98, K=0.5, seed=1):
+    """-> rows {L, ms_per_mcs, updates_per_s, hours_per_1e6_mcs, rho_C}."""
+    import torch
+    rows = []
+    stream = torch.cuda.current_stream()
+    for L in Ls:
+        d = torch.empty((L, L), dtype=torch.uint8, device="cuda")
+        cnt = torch.zeros(n_mcs, dtype=torch.int64, device="cuda")
+        pgg_init_lattice(d, FMT_U8, L, 0.5, seed, stream)
+        pgg_sweep(d, FMT_U8, L, r, K, seed, order, 0, n_mcs, None, stream)       # warm-up, reaches rho_C ~ 0.5
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        pgg_sweep(d, FMT_U8, L, r, K, seed, order, n_mcs, n_mcs, cnt, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / n_mcs
+        rows.append({"L": L, "ms_per_mcs": ms, "updates_per_s": L * L / (ms * 1e-3),
+                     "hours_per_1e6_mcs": ms * 1e3 / 3600.0, "rho_C": float(cnt[-1]) / (L * L)})
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("what", choices=["stationary", "decay"])
+    ap.add_argument("what", choices=["stationary", "decay", "fig5"])
     ap.add_argument("--L", type=int, default=0)
     ap.add_argument("--mcs", type=int, default=0)
     ap.add_argument("--seeds", type=int, nargs="+", default=None)
-    ap.add_argument("--order", default="iid", choices=["iid", "perm"])
+    ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"])
     ap.add_argument("--rs", type=float, nargs="+", default=None)
     ap.add_argument("--r", type=float, default=3.7443)
     args = ap.parse_args()
-    order = ORDER_IID if args.order == "iid" else ORDER_PERM
-    if args.what == "stationary":
+    order = {"iid": ORDER_IID, "perm": ORDER_PERM, "dtile": ORDER_DTILE}[args.order]
+    if args.what == "fig5":
+        print(json.dumps({"what": "fig5", "order": args.order, "r": 3.98, "mcs_timed": args.mcs or 2000,
+                          "rows": fig5(order, args.mcs or 2000)}))
+    elif args.what == "stationary":
         rs = args.rs or [round(3.60 + 0.05 * a, 2) for a in range(9)] + [5.3, 5.4, 5.5, 5.6]
         res = stationary(rs, args.seeds or [101, 102, 103, 104], args.L or 400, args.mcs or 20000, order=order)
         print(json.dumps({"what": "stationary", "order": args.order, "L": args.L or 400, "mcs": args.mcs or 20000,
