@@ -64,9 +64,17 @@ constexpr unsigned long long dtile_bits(std::initializer_list<int> offs)
 constexpr unsigned long long kDtileW2 = dtile_bits({-1, 1, -12, 12, -13, -11, 11, 13});
 constexpr unsigned long long kDtileW1 = dtile_bits({-2, 2, -24, 24});
 __device__ __forceinline__ int dtile_s(unsigned long long w) { return (int)((w >> kDtileCentre) & 1ull); }
-__device__ __forceinline__ int dtile_A(unsigned long long w)
+// 2 (nearest + diagonal) + axial distance-2 of the centre site, i.e. A - 5 s.  The weight-2 bits span
+// 27 positions (centre -13 .. +13) and the weight-1 bits fold into one word without colliding (bits
+// 2, 24, 28 and 50 - 32 = 18), so each sum is ONE 32-bit population count (POPC issues at a fraction
+// of the ALU rate).
+__device__ __forceinline__ int dtile_nbsum(unsigned long long w)
 {
-    return 5 * dtile_s(w) + 2 * __popcll(w & kDtileW2) + __popcll(w & kDtileW1);
+    static_assert(kDtileCentre == 26, "the folding below assumes the centre at bit 26");
+    const uint32_t w2 = (uint32_t)(w >> 13) & (uint32_t)(kDtileW2 >> 13);
+    const unsigned long long a = w & kDtileW1;
+    const uint32_t w1 = (uint32_t)a | (uint32_t)(a >> 32);
+    return 2 * __popc(w2) + __popc(w1);
 }
 
 // The 12 sites of lattice row i starting at column c0 (a multiple of 4, may be -4), periodic,
@@ -162,7 +170,7 @@ dtile_part_kernel(PhaseArgs a, uint32_t m, uint32_t q)
             const unsigned long long wx = P.window(pr, pc), wy = P.window(yr, yc);
             const int sx = dtile_s(wx), sy = dtile_s(wy);
             // branch-free: with 32 live domains per warp some lane nearly always needs the payoffs
-            const int dA = dtile_A(wx) - dtile_A(wy);
+            const int dA = 5 * (sx - sy) + dtile_nbsum(wx) - dtile_nbsum(wy);
             const uint32_t T = table[table_index(dA, sx - sy)];
             if (sx != sy && x[1] < T) P.toggle(pr, pc);
         }
