@@ -46,3 +46,13 @@ def test_bench_reference_arm_line():
     d = json.loads([ln for ln in p.stdout.splitlines() if ln.startswith("{")][0])
     assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+
+
+def test_bench_line_for_the_papers_schedule():
+    """--order dtile: same contract line, 4 launches per MCS, no class-order kernel."""
+    d = run_bench("--order", "dtile", "--no-cpu-baseline")
+    assert d["config"]["order_mode"] == "dtile" and d["config"]["variant"] == 10
+    assert d["gpu_launches"] == 2 * (1 + 1 + 4 * 20 + 1)
+    r = d["roofline"]
+    assert r["algorithmic_bytes_per_launch"] == 1024 * 1024 * 1.25 and "dtile_part_kernel" in r["kernel"]
+    assert d["value"] > 0 and d["e2e"]["value"] > 0 and 0.0 <= d["final_rho_C"] <= 1.0
