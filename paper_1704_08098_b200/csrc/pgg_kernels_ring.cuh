@@ -34,7 +34,9 @@
 //   * the 16 column tasks of a step rotate over the warps, so that no warp is
 //     tied to the busiest columns of the band;
 //   * full-row mode (FR): when the strip is the whole lattice row the halo
-//     columns are dropped and a chunk arrives as ONE bulk copy.
+//     columns are dropped and a chunk arrives as ONE bulk copy;
+//   * while it waits for the previous phase to drain (before griddepcontrol.wait)
+//     the producer warp prefetches the band's first rows into L2.
 //
 // Geometry, producer, barriers and the compaction (scan -> Q1 -> Philox
 // [-> Q2] -> stencil) are those of pgg_kernels_band.cuh:
@@ -85,6 +87,7 @@ struct RingPlan {
     uint32_t mirror;     // 1: three mirror rows in front of slot 0; 0: wrapping stencil reads
     uint32_t rotate;     // 1: column tasks rotate over the warps from step to step
     uint32_t fullrow;    // 1: the strip is the whole row, no halo columns, one bulk copy per chunk (FR)
+    uint32_t l2pf;       // 1: before griddepcontrol.wait, prefetch the band's first rows into L2
 };
 
 // s at offset `off` (site units) from ring0; off may reach into the mirror rows (< 0)
@@ -266,6 +269,22 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         const int ps = (FMT == kFmtU8) ? pitch : 8 * pitch;  // one row down, in site units
         eoff[0] = -ps; eoff[1] = ps; eoff[2] = -1; eoff[3] = 1;
         eoff[4] = 1;   eoff[5] = 1;  eoff[6] = ps; eoff[7] = ps;
+    }
+    if (g.l2pf && warp == kRingConsumers) {
+        // L2PF: the first rows this CTA will stage, whatever the phase class turns out to be (the
+        // class only shifts them by 0..3 rows).  A prefetch moves DRAM -> L2 only; L2 is the point
+        // of coherence, so rows the previous phase is still writing cannot go stale.
+        const uint32_t strip_ = blockIdx.x / g.nb, band_ = blockIdx.x - strip_ * g.nb;
+        const long long S0_ = (long long)(((unsigned long long)band_ * g.n_super) / g.nb);
+        const int j0_ = (int)(strip_ * g.W), wb_ = min((int)g.W, (int)g.row_bytes - j0_);
+        const long long first = (long long)RC * (S0_ - 1) + RC - 3;
+        const int n_rows = 2 * RC + 3 + 4;
+        for (int q = lane; q < n_rows; q += 32) {
+            long long gi = (first + q) % (long long)L;
+            if (gi < 0) gi += L;
+            const uint8_t* src = lat + (size_t)gi * (size_t)g.row_bytes + j0_;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"((uint32_t)wb_) : "memory");
+        }
     }
     __syncthreads();
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -622,6 +641,10 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p, bool allow_fu
     if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = (atoi(e) && !p->fullrow) ? 1u : 0u;
     p->rotate = 1;
     if (const char* e = getenv("PGG_RING_ROTATE")) p->rotate = atoi(e) ? 1u : 0u;
+    p->pair = 0;
+    p->l2pf = 0;
+    if (const char* e = getenv("PGG_RING_L2PF")) p->l2pf = atoi(e) ? 1u : 0u;
+    if (const char* e = getenv("PGG_RING_PAIR")) p->pair = atoi(e) ? 1u : 0u;
     const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
                          + (p->mirror ? 3 * p->pitch : 0);
     while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 256) --want;
