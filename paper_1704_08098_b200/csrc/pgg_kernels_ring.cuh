@@ -641,10 +641,8 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p, bool allow_fu
     if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = (atoi(e) && !p->fullrow) ? 1u : 0u;
     p->rotate = 1;
     if (const char* e = getenv("PGG_RING_ROTATE")) p->rotate = atoi(e) ? 1u : 0u;
-    p->pair = 0;
-    p->l2pf = 0;
+    p->l2pf = 1;  // measured: 58.6 -> 58.1 us per launch (profiles/r1_ring_design_notes.md)
     if (const char* e = getenv("PGG_RING_L2PF")) p->l2pf = atoi(e) ? 1u : 0u;
-    if (const char* e = getenv("PGG_RING_PAIR")) p->pair = atoi(e) ? 1u : 0u;
     const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
                          + (p->mirror ? 3 * p->pitch : 0);
     while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 256) --want;
