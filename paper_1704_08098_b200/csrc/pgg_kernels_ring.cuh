@@ -87,7 +87,7 @@ struct RingPlan {
     uint32_t mirror;     // 1: three mirror rows in front of slot 0; 0: wrapping stencil reads
     uint32_t rotate;     // 1: column tasks rotate over the warps from step to step
     uint32_t fullrow;    // 1: the strip is the whole row, no halo columns, one bulk copy per chunk (FR)
-    uint32_t l2pf;       // 1: before griddepcontrol.wait, prefetch the band's first rows into L2
+    uint32_t l2pf;       // n > 0: before griddepcontrol.wait, prefetch the band's first n chunks into L2
 };
 
 // s at offset `off` (site units) from ring0; off may reach into the mirror rows (< 0)
@@ -278,7 +278,7 @@ phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
         const long long S0_ = (long long)(((unsigned long long)band_ * g.n_super) / g.nb);
         const int j0_ = (int)(strip_ * g.W), wb_ = min((int)g.W, (int)g.row_bytes - j0_);
         const long long first = (long long)RC * (S0_ - 1) + RC - 3;
-        const int n_rows = 2 * RC + 3 + 4;
+        const int n_rows = ((int)g.l2pf - 1) * RC + 3 + 4;  // the tail of chunk 0 and l2pf - 1 whole chunks, + 4 for the class
         for (int q = lane; q < n_rows; q += 32) {
             long long gi = (first + q) % (long long)L;
             if (gi < 0) gi += L;
@@ -641,8 +641,8 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p, bool allow_fu
     if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = (atoi(e) && !p->fullrow) ? 1u : 0u;
     p->rotate = 1;
     if (const char* e = getenv("PGG_RING_ROTATE")) p->rotate = atoi(e) ? 1u : 0u;
-    p->l2pf = 1;  // measured: 58.6 -> 58.1 us per launch (profiles/r1_ring_design_notes.md)
-    if (const char* e = getenv("PGG_RING_L2PF")) p->l2pf = atoi(e) ? 1u : 0u;
+    p->l2pf = 3;  // chunks; measured: 58.6 -> 58.1 us per launch (profiles/r1_ring_design_notes.md)
+    if (const char* e = getenv("PGG_RING_L2PF")) p->l2pf = (uint32_t)std::max(0, std::min(64, atoi(e)));
     const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
                          + (p->mirror ? 3 * p->pitch : 0);
     while (want > 3 && want * p->slot_bytes + fixed > (uint32_t)smem_optin - 256) --want;
