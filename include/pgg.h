@@ -143,7 +143,8 @@ int32_t pgg_run_ensemble(void* d_lats, int32_t fmt, uint32_t B, uint32_t L, cons
 
 /* The 16 phase classes of MCS t, computed by the library's own
  * device kernel and copied back; h_out16: host array of 16 bytes.  Synchronises
- * `stream`.  For tests of step a1.                                               */
+ * `stream`.  For tests of step a1.  PGG_ORDER_DTILE has no classes:
+ * PGG_ERR_UNSUPPORTED.                                                           */
 int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t* h_out16,
                           void* stream);
 

@@ -73,6 +73,10 @@ def test_argument_validation_returns_error_codes():
     assert h.pgg_sweep(fake, 0, 64, 4.0, 0.5, 1, 9, 0, 1, None, None) == pgg.ERR_UNSUPPORTED
     assert h.pgg_sweep(fake, 0, 64, 4.0, 0.5, 1, 0, 2**32 - 1, 2, None, None) == pgg.ERR_BAD_PARAM
     assert h.pgg_density(fake, 0, 64, None, None) == pgg.ERR_NULL
+    # the paper's double-tiling schedule needs L % 8 == 0 and has no phase classes
+    assert h.pgg_sweep(fake, 0, 12, 4.0, 0.5, 1, pgg.ORDER_DTILE, 0, 1, None, None) == pgg.ERR_BAD_L
+    assert h.pgg_sweep(fake, 0, 64, 4.0, 0.0, 1, pgg.ORDER_DTILE, 0, 1, None, None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_set_variant(10) == pgg.ERR_UNSUPPORTED  # PGG_VARIANT_DTILE is reported, not selectable
     r = (C.c_double * 1)(4.0)
     s = (C.c_uint64 * 1)(1)
     assert h.pgg_run_ensemble(fake, 0, 0, 64, r, 0.5, s, 0, 0.5, 0, 1, None, None) == pgg.ERR_BAD_PARAM
