@@ -75,7 +75,7 @@ enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
 
 /* Kernel variants of the phase step (all bit-identical).
  * PGG_VARIANT_AUTO picks by measurement (profiles/r1_ring_design_notes.md):
- * RESIDENT for L <= 320 or many lattices (B L^2 >= 32 * 512^2, L <= 512); RING
+ * RESIDENT for L <= 320 or many lattices (B L^2 >= 16 * 512^2, L <= 512); RING
  * (uint8) / BAND (bit-packed) for L >= 2048 and for uint8 L = 512, 1024; else V0. */
 enum {
     PGG_VARIANT_AUTO = 0,

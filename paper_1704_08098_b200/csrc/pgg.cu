@@ -156,7 +156,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         // RESIDENT takes one SM per lattice whatever B is, and its time grows with L^2 (1.5 us per
         // phase at L = 64, 7-13 at L = 512); a per-phase launch costs 4-5 us until B L^2 makes it
         // throughput-bound (L = 512: V0 6 us at B = 8, 24 at B = 64).  So: small lattices, or many.
-        const bool res_pays = L <= 320 || (unsigned long long)B * L * L >= 32ull * 512ull * 512ull;
+        const bool res_pays = L <= 320 || (unsigned long long)B * L * L >= 16ull * 512ull * 512ull;
         // the streaming kernels need long rows (or whole-row strips: uint8 L = 512 * 2^k) to beat
         // V0's launch-bound 4-5 us; below that their fixed cost is ~9.5 us per launch
         const bool stream_pays = L >= 2048 || (fmt == PGG_FMT_U8 && L >= 512 && (L & (L - 1)) == 0);
