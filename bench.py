@@ -176,7 +176,7 @@ def run_ours(args):
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
                "fused": pgg.VARIANT_FUSED, "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND,
-               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT}[args.variant]
+               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT, "lean": pgg.VARIANT_LEAN}[args.variant]
     pgg.pgg_set_variant(variant)
     seed = SEED + rank
     shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
@@ -267,6 +267,15 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
+    # ---- the ALU ceiling: STEP draws per second of a Philox-only kernel
+    n_draws = pgg.pgg_probe_draw_rate(64, seed, stream)          # warm-up launch
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(stream)
+    n_draws = sum(pgg.pgg_probe_draw_rate(2048, seed, stream) for _ in range(4))
+    p1.record(stream)
+    stream.synchronize()
+    draws_per_s = n_draws / (p0.elapsed_time(p1) * 1e-3)
+
     # ---- roofline of the dominant kernel (the phase kernel; 16 launches per MCS)
     peak, peak_src = load_peaks()
     # (the paper's double-tiling schedule, --order dtile: 4 parts per MCS, each reads N and writes N/4)
@@ -314,6 +323,10 @@ def run_ours(args):
                 "d2h_bytes_per_step": lat_bytes + 8 * n_mcs, "steps": e2e_steps,
                 "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": e2e_wall_ms / e2e_steps},
         "roofline": roofline,
+        "ceilings": {"philox_step_draws_per_s": draws_per_s,
+                     "note": "pgg_probe_draw_rate: every thread of a full grid makes STEP draws only "
+                             "(Philox4x32-10, words x0/x1, two chains per thread); the rate no phase kernel "
+                             "can exceed for the sites that need a draw (SURVEY 8(d)(ii))"},
     }
     if world == 1 and not args.no_cpu_baseline:
         v, threads, n_done, dt = oracle_sample(L, max_mcs=8, min_seconds=10.0)
@@ -335,7 +348,7 @@ def main():
     ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
-    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band", "ring", "split", "dyn", "resident"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "fused", "pipe", "band", "ring", "split", "dyn", "resident", "lean"])
     ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"],
                     help="schedule: the 16-sublattice schedule with i.i.d. (bench default) or permuted classes, or "
                          "the paper's own double-tiling schedule (PAPER.md:75-93); anything but iid is not the bench workload")

@@ -44,7 +44,8 @@ extern "C" {
 enum {
     PGG_OK = 0,
     PGG_ERR_NULL = -1,        /* a required pointer is NULL                              */
-    PGG_ERR_BAD_L = -2,       /* L < 4, L % 4 != 0, L > 65536, or (bits) L % 32 != 0     */
+    PGG_ERR_BAD_L = -2,       /* L < 4, L % 4 != 0, L >= 65536 (site indices are uint32: every
+                                 entry point, pgg_density included), or (bits) L % 32 != 0 */
     PGG_ERR_BAD_PARAM = -3,   /* r/K not finite, K <= 0, rho0 outside [0,1], B == 0, ... */
     PGG_ERR_ALIGN = -4,       /* lattice pointer not 16-byte aligned                     */
     PGG_ERR_UNSUPPORTED = -5, /* unknown fmt / order_mode / kernel variant               */
@@ -89,8 +90,10 @@ enum {
     PGG_VARIANT_DYN = 8,  /* RING with dynamically assigned tasks, 24 warps (uint8)   */
     PGG_VARIANT_RESIDENT = 9,/* L <= 512: one CTA per lattice, lattice resident in smem,
                                 every phase of the call in one launch                  */
-    PGG_VARIANT_DTILE = 10   /* reported by pgg_get_variant_used() after a PGG_ORDER_DTILE
+    PGG_VARIANT_DTILE = 10,  /* reported by pgg_get_variant_used() after a PGG_ORDER_DTILE
                                 sweep (one thread per 4x4 domain); not selectable       */
+    PGG_VARIANT_LEAN = 11    /* L = 1024 .. 32768, a power of two: whole rows streamed, packed to
+                                bits on arrival (uint8), scan / draw / stencil on a bit ring   */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:
@@ -156,6 +159,14 @@ int32_t pgg_get_variant_used(void);
 
 /* 1 if kernel variant `variant` can run lattices of layout fmt and size L, else 0. */
 int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L);
+
+/* ALU ceiling probe ("a Philox-only kernel's site-draws/s").  Enqueues ONE
+ * launch of a kernel in which every thread of a full grid makes 2*iters STEP draws (the draw
+ * of an elementary step, exactly as the phase kernels compute it: Philox4x32-10,
+ * counter (site, t, (k<<8)|c, 3), words x0 and x1) and nothing else.  *h_n_draws (host, written
+ * before return) = draws the launch makes; the caller times the launch with events on `stream`.
+ * No lattice is touched.  Errors: PGG_ERR_NULL, PGG_ERR_BAD_PARAM (iters == 0), PGG_ERR_CUDA. */
+int32_t pgg_probe_draw_rate(uint32_t iters, uint64_t seed, uint64_t* h_n_draws, void* stream);
 
 /* Number of kernels this library has launched in this process (monotone).       */
 uint64_t pgg_launch_count(void);

@@ -22,6 +22,7 @@ ERR_NULL, ERR_BAD_L, ERR_BAD_PARAM, ERR_ALIGN, ERR_UNSUPPORTED, ERR_CUDA = -1, -
 FMT_U8, FMT_BITS = 0, 1
 ORDER_IID, ORDER_PERM, ORDER_DTILE = 0, 1, 2
 VARIANT_AUTO, VARIANT_V0, VARIANT_TILE, VARIANT_FUSED, VARIANT_PIPE, VARIANT_BAND, VARIANT_RING, VARIANT_SPLIT, VARIANT_DYN, VARIANT_RESIDENT = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
+VARIANT_DTILE, VARIANT_LEAN = 10, 11
 
 # name -> (restype, argtypes); also the list of symbols include/pgg.h declares
 _u32p, _u64p, _u8p, _f64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_uint8),
@@ -40,6 +41,7 @@ SIGNATURES = {
     "pgg_set_variant": (C.c_int32, [C.c_int32]),
     "pgg_get_variant_used": (C.c_int32, []),
     "pgg_variant_supported": (C.c_int32, [C.c_int32, C.c_int32, C.c_uint32]),
+    "pgg_probe_draw_rate": (C.c_int32, [C.c_uint32, C.c_uint64, _u64p, C.c_void_p]),
     "pgg_launch_count": (C.c_uint64, []),
     "pgg_last_error": (C.c_char_p, []),
 }
@@ -130,6 +132,13 @@ def pgg_get_variant_used() -> int:
 
 def pgg_variant_supported(variant: int, fmt: int, L: int) -> bool:
     return bool(lib().pgg_variant_supported(variant, fmt, L))
+
+
+def pgg_probe_draw_rate(iters: int, seed: int = 1, stream=None) -> int:
+    """Enqueue one launch of the Philox-only probe; -> number of STEP draws it makes."""
+    n = C.c_uint64(0)
+    _check(lib().pgg_probe_draw_rate(iters, seed, C.byref(n), _stream(stream)))
+    return int(n.value)
 
 
 def pgg_launch_count() -> int:

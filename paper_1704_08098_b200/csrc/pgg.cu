@@ -22,7 +22,9 @@
 #include "pgg_kernels_split.cuh"
 #include "pgg_kernels_dyn.cuh"
 #include "pgg_kernels_resident.cuh"
+#include "pgg_kernels_lean.cuh"
 #include "pgg_kernels_dtile.cuh"
+#include "pgg_kernels_probe.cuh"
 
 namespace {
 
@@ -60,8 +62,8 @@ int32_t check_lattice_args(const void* d_lat, int32_t fmt, uint32_t L)
 {
     if (d_lat == nullptr) return fail(PGG_ERR_NULL, "lattice pointer is NULL");
     if (fmt != PGG_FMT_U8 && fmt != PGG_FMT_BITS) return fail(PGG_ERR_UNSUPPORTED, "unknown fmt %d", fmt);
-    if (L < 4 || L % 4 != 0 || L > 65536)
-        return fail(PGG_ERR_BAD_L, "L = %u: need 4 <= L <= 65536 and L %% 4 == 0", L);
+    if (L < 4 || L % 4 != 0 || L >= 65536)  // site indices (Philox counter word, uint32) need L*L <= 2^32 - 1
+        return fail(PGG_ERR_BAD_L, "L = %u: need 4 <= L <= 65532 and L %% 4 == 0", L);
     if (fmt == PGG_FMT_BITS && L % 32 != 0)
         return fail(PGG_ERR_BAD_L, "L = %u: the bit-packed layout needs L %% 32 == 0", L);
     if ((reinterpret_cast<uintptr_t>(d_lat) & 15u) != 0)
@@ -97,8 +99,7 @@ int32_t launch_init(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, double
 {
     // thr = floor(rho0 * 2^32) in [0, 2^32]  (D4)
     const unsigned long long thr = (unsigned long long)std::floor(rho0 * 4294967296.0);
-    const uint32_t n_sites = L * L;  // L <= 65536: L*L may be 2^32 -> handled below
-    if (L == 65536) return fail(PGG_ERR_BAD_L, "L = 65536: site index does not fit the init counter");
+    const uint32_t n_sites = L * L;  // L <= 65532 (check_lattice_args)
     const unsigned long long lb = lattice_bytes(fmt, L);
     const uint32_t n_items = fmt == PGG_FMT_U8 ? n_sites >> 4 : n_sites >> 5;
     uint32_t gx = (n_items + 255) / 256;
@@ -143,7 +144,6 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         if (!std::isfinite(h_r[b])) return fail(PGG_ERR_BAD_PARAM, "r[%u] is not finite", b);
     if ((unsigned long long)t_begin + n_mcs > 4294967296ull)
         return fail(PGG_ERR_BAD_PARAM, "t_begin + n_mcs exceeds 2^32");
-    if (L == 65536) return fail(PGG_ERR_BAD_L, "L = 65536: site index does not fit uint32 counters");
 
     int variant = order_mode == PGG_ORDER_DTILE ? PGG_VARIANT_DTILE : g_variant.load();
     const bool tile_ok = pgg::tile_supported(fmt, L);
@@ -160,11 +160,17 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         // the streaming kernels need long rows (or whole-row strips: uint8 L = 512 * 2^k) to beat
         // V0's launch-bound 4-5 us; below that their fixed cost is ~9.5 us per launch
         const bool stream_pays = L >= 2048 || (fmt == PGG_FMT_U8 && L >= 512 && (L & (L - 1)) == 0);
+        // bit-packed: LEAN (rows stream into a bit ring, queue lifetime of several steps) measured 2-3x
+        // faster than BAND on ensembles and sparse states and level with it on the dense C5 lattice
+        const bool lean_bits = fmt == PGG_FMT_BITS && pgg::lean_supported(fmt, L);
         variant = (res_ok && res_pays) ? PGG_VARIANT_RESIDENT
+                : lean_bits ? PGG_VARIANT_LEAN
                 : !stream_pays ? PGG_VARIANT_V0
                 : (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
     }
     if (variant == PGG_VARIANT_RESIDENT && !res_ok)
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
+    if (variant == PGG_VARIANT_LEAN && !pgg::lean_supported(fmt, L))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     const bool split_ok = pgg::split_supported(fmt, L);
     if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
@@ -273,6 +279,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         if (rc != 0) return fail(PGG_ERR_CUDA, "tile kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
     }
 
+    pgg::LeanPlan lplan;
+    if (variant == PGG_VARIANT_LEAN) {
+        int32_t rc = pgg::lean_plan(fmt, L, B, &lplan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "lean kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
     pgg::ResPlan resplan;
     if (variant == PGG_VARIANT_RESIDENT) {
         int32_t rc = pgg::resident_plan(fmt, L, &resplan);
@@ -290,7 +301,9 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         }
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
-                if (variant == PGG_VARIANT_DYN) {
+                if (variant == PGG_VARIANT_LEAN) {
+                    pgg::lean_launch(lplan, fmt, a, m, k, B, stream);
+                } else if (variant == PGG_VARIANT_DYN) {
                     pgg::dyn_launch(rplan, a, m, k, B, stream);
                 } else if (variant == PGG_VARIANT_SPLIT) {
                     pgg::split_launch(rplan, a, m, k, B, stream);
@@ -413,7 +426,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_RESIDENT)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_LEAN || variant == PGG_VARIANT_DTILE)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -432,7 +445,27 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_SPLIT) return pgg::split_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_DYN) return pgg::dyn_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_RESIDENT) return pgg::resident_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_LEAN) return pgg::lean_supported(fmt, L) ? 1 : 0;
     return 0;
+}
+
+int32_t pgg_probe_draw_rate(uint32_t iters, uint64_t seed, uint64_t* h_n_draws, void* stream)
+{
+    if (h_n_draws == nullptr) return fail(PGG_ERR_NULL, "h_n_draws is NULL");
+    if (iters == 0) return fail(PGG_ERR_BAD_PARAM, "iters must be > 0");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 0;
+    PGG_CUDA(cudaGetDevice(&dev));
+    PGG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const uint32_t grid = (uint32_t)sms * 4u;  // 4 CTAs of 256 threads per SM: every SM full at 64 registers
+    Scratch tmp(s);
+    uint32_t* d_sink = nullptr;
+    PGG_CUDA(tmp.alloc((void**)&d_sink, sizeof(uint32_t) * grid * pgg::kProbeThreads));
+    const pgg::StepKey sk = pgg::make_step_key(seed, 0u, 0u, 0u);
+    pgg::draw_ceiling_kernel<<<grid, pgg::kProbeThreads, 0, s>>>(sk, iters, d_sink);
+    PGG_LAUNCHED();
+    *h_n_draws = 2ull * iters * grid * pgg::kProbeThreads;
+    return PGG_OK;
 }
 
 uint64_t pgg_launch_count(void) { return g_launches.load(); }

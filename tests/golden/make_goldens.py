@@ -79,9 +79,9 @@ def main():
     if args.config == "c2":      # BASELINE.json configs[1], one seed, full length
         cfg = wl.config2(seed=101, n_mcs=args.mcs or 20000)
         snaps = [cfg.n_mcs // 2, cfg.n_mcs]
-    elif args.config == "c3":    # configs[2]: prefix of the 10^5 MCS (full: ~100 core hours)
-        cfg = wl.config3(n_mcs=args.mcs or 1000)
-        snaps = [cfg.n_mcs]
+    elif args.config == "c3":    # configs[2]: a prefix for all 16 seeds, or the full 10^5 MCS for a few
+        cfg = wl.config3(n_mcs=args.mcs or 1000)   # (--mcs 100000 --members 2: ~6 core hours per seed)
+        snaps = [cfg.n_mcs] if cfg.n_mcs < 10000 else [cfg.n_mcs // 10, cfg.n_mcs // 2, cfg.n_mcs]
     elif args.config == "c4":    # configs[3], full length
         cfg = wl.config4(n_mcs=args.mcs or 10000)
         snaps = [cfg.n_mcs // 10, cfg.n_mcs]
@@ -90,7 +90,9 @@ def main():
         snaps = sorted({2, cfg.n_mcs // 10, cfg.n_mcs // 3, cfg.n_mcs})
     B = args.members or cfg.batch
     solo = B == 1
-    jobs = [(cfg.L, cfg.rs[b], cfg.K, cfg.rho0, cfg.seeds[b], cfg.n_mcs, snaps, procs if solo else 1)
+    # threads per lattice: all of them for one lattice, else what is left per pool process
+    per_member = procs if solo else max(1, procs // B)
+    jobs = [(cfg.L, cfg.rs[b], cfg.K, cfg.rho0, cfg.seeds[b], cfg.n_mcs, snaps, per_member)
             for b in range(B)]
     t0 = time.time()
     if solo:

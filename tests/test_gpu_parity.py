@@ -17,7 +17,7 @@ import paper_1704_08098_b200 as pgg  # noqa: E402
 K = wl.K_DEFAULT
 FMTS = [pgg.FMT_U8, pgg.FMT_BITS]
 VARIANTS = [pgg.VARIANT_V0, pgg.VARIANT_TILE, pgg.VARIANT_PIPE, pgg.VARIANT_BAND, pgg.VARIANT_RING, pgg.VARIANT_SPLIT, pgg.VARIANT_DYN,
-            pgg.VARIANT_RESIDENT]
+            pgg.VARIANT_RESIDENT, pgg.VARIANT_LEAN]
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -380,3 +380,144 @@ def test_large_lattice_L32768():
     del d
     assert np.array_equal(got, ref), "L=32768 lattice differs"
     assert int(cnt.item()) == int(ref_counts[0])
+
+
+# ---------------------------------------------------------------- long calls: order-buffer chunks, late windows
+# run_sweeps() holds the phase classes of at most 4096 MCS on the device and rewrites that buffer
+# between two dependent-launch chained phases; every 10^5..10^6-MCS physics run crosses it.
+LONG_CASES = [
+    # (variant, fmt, L, env) -- the kernels AUTO ships for long runs, each forced by name
+    ("RING", pgg.FMT_U8, 512, {}),                               # RING, full-row mode (C3's path)
+    ("RING", pgg.FMT_U8, 512, {"PGG_RING_FULLROW": "0"}),        # RING, strips with halo columns (C5's path)
+    ("BAND", pgg.FMT_BITS, 512, {}),                             # BAND, bit-packed (C5 packed)
+    ("LEAN", pgg.FMT_U8, 1024, {}),                              # LEAN, uint8 packed to bits on chip
+    ("LEAN", pgg.FMT_BITS, 1024, {}),                            # LEAN, bit-packed source
+]
+
+
+def _variant_by_name(name):
+    return getattr(pgg, "VARIANT_" + name)
+
+
+@pytest.mark.parametrize("name,fmt,L,env", LONG_CASES,
+                         ids=[f"{n}-{'u8' if f == pgg.FMT_U8 else 'bits'}-L{L}{'-strips' if e else ''}"
+                              for n, f, L, e in LONG_CASES])
+def test_one_call_longer_than_an_order_chunk(name, fmt, L, env, monkeypatch):
+    """ONE call of 4200 MCS from t_begin = 4000 (a call that starts mid-way through the run and
+    crosses the 4096-MCS order-buffer boundary): lattice and the whole count trace against a live
+    oracle run.  PAPER.md:113 (runs of 10^5..3*10^6 MCS near r_c) is what takes this path."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    use_variant(_variant_by_name(name), fmt, L)
+    seed, r, t0, n_mcs = 900 + L, 3.8, 4000, 4200
+    lat0 = orc.init(L, 0.5, seed)
+    ref = lat0.copy()
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, t0, n_mcs, n_threads=orc.max_threads())
+    got, counts = gpu_sweep(lat0, fmt, r, seed, pgg.ORDER_IID, t0, n_mcs)
+    assert_same(counts, ref_counts, "count trace across the chunk boundary")
+    assert_same(got, ref, "lattice after 4200 MCS")
+    assert 0 < int(ref_counts[-1]) < L * L, "the run must not have been absorbed (it would test nothing)"
+
+
+@pytest.mark.parametrize("name,fmt,L,env", LONG_CASES,
+                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits"])
+@pytest.mark.parametrize("t0", [99900, 2**32 - 40])
+def test_streaming_kernels_late_windows(name, fmt, L, env, t0, monkeypatch):
+    """SURVEY 8(d) late windows (t = 99 900) and the counter width (t_begin + m up to 2^32 - 1)
+    for the streaming kernels by name; the oracle starts from the same given state (legal by P7)."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    use_variant(_variant_by_name(name), fmt, L)
+    seed, r, n_mcs = 2**34 + 77, 3.9, 40
+    lat0 = wl.random_lattice(L, 0.3, 5)
+    ref = lat0.copy()
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, t0, n_mcs, n_threads=orc.max_threads())
+    got, counts = gpu_sweep(lat0, fmt, r, seed, pgg.ORDER_IID, t0, n_mcs)
+    assert_same(got, ref, f"lattice, window at t = {t0}")
+    assert_same(counts, ref_counts, f"counts, window at t = {t0}")
+
+
+# ---------------------------------------------------------------- LEAN (L = 1024 .. 32768, powers of two)
+@pytest.mark.parametrize("fmt", FMTS)
+@pytest.mark.parametrize("L,n_mcs", [(1024, 6), (2048, 4), (4096, 3), (8192, 2)])
+def test_lean_parity_sizes(fmt, L, n_mcs):
+    """One band per SM down to one step per CTA (L = 1024: 16 active rows per step), both orders,
+    a 64-bit seed, from the dense random start (every extraction round crowded) and a sparse one."""
+    use_variant(pgg.VARIANT_LEAN, fmt, L)
+    for seed, r, order, rho0 in ((L + 1, 3.8, pgg.ORDER_IID, 0.5), (2**35 + L, 4.6, pgg.ORDER_PERM, 0.1)):
+        lat0 = orc.init(L, rho0, seed)
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, r, K, seed, order, 3, n_mcs, n_threads=orc.max_threads())
+        got, counts = gpu_sweep(lat0, fmt, r, seed, order, 3, n_mcs)
+        assert pgg.pgg_get_variant_used() == pgg.VARIANT_LEAN
+        assert_same(got, ref, f"lattice L={L}")
+        assert_same(counts, ref_counts, f"counts L={L}")
+
+
+@pytest.mark.parametrize("fmt", FMTS)
+def test_lean_structured_absorbing_and_clamped(fmt):
+    """Checkerboard (all eight active sites of every word survive the S9 test: the split
+    extraction round), stripes and blobs (mostly bulk), absorbing states, clamped tables."""
+    L = 1024
+    use_variant(pgg.VARIANT_LEAN, fmt, L)
+    states = [wl.checkerboard_lattice(L), wl.stripes_lattice(L, 5, True), wl.stripes_lattice(L, 7, False),
+              wl.blobs_lattice(L, 3), wl.random_lattice(L, 0.03, 8), wl.random_lattice(L, 0.97, 9)]
+    for n, lat0 in enumerate(states):
+        for r, Kx in ((3.8, K), (5.4, K), (4.0, 1e-3)):
+            ref = lat0.copy()
+            ref_counts, _ = orc.sweep(ref, r, Kx, 77 + n, pgg.ORDER_IID, 0, 4, n_threads=orc.max_threads())
+            d = to_device(lat0, fmt)
+            cnt = torch.zeros(4, dtype=torch.int64, device="cuda")
+            pgg.pgg_sweep(d, fmt, L, r, Kx, 77 + n, pgg.ORDER_IID, 0, 4, cnt)
+            torch.cuda.synchronize()
+            assert_same(to_host(d, fmt, L), ref, f"state {n} r={r} K={Kx}")
+            assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts, f"counts state {n}")
+    for v in (0, 1):
+        lat0 = np.full((L, L), v, dtype=np.uint8)
+        got, counts = gpu_sweep(lat0, fmt, 3.8, 5, pgg.ORDER_IID, 0, 3)
+        assert_same(got, lat0)
+        assert (counts == v * L * L).all()
+
+
+@pytest.mark.parametrize("fmt", FMTS)
+def test_lean_ensemble_equals_solo_and_oracle(fmt):
+    """Config-3 shape at reduced length: B lattices of L = 2048 in one grid per phase (bands share
+    the SMs), each with its own r and seed; then continued (rho0 < 0) in PERM order."""
+    B, L, n_mcs = 5, 2048, 3
+    use_variant(pgg.VARIANT_LEAN, fmt, L)
+    rs = [3.74 + 0.01 * b for b in range(B)]
+    seeds = [2**33 + 11 * b for b in range(B)]
+    d = empty_lattice(fmt, L, B)
+    cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, n_mcs, cnt)
+    torch.cuda.synchronize()
+    got = to_host(d, fmt, L)
+    for b in range(B):
+        ref = orc.init(L, 0.5, seeds[b])
+        ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs, n_threads=orc.max_threads())
+        assert_same(got[b], ref, f"member {b}")
+        assert_same(cnt[b].cpu().numpy().astype(np.uint64), ref_counts)
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_PERM, -1.0, n_mcs, 2, None)
+    torch.cuda.synchronize()
+    got2 = to_host(d, fmt, L)
+    for b in (0, B - 1):
+        ref = got[b].copy()
+        orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_PERM, n_mcs, 2, n_threads=orc.max_threads())
+        assert_same(got2[b], ref, f"member {b} continued")
+
+
+@pytest.mark.parametrize("fmt", FMTS)
+def test_lean_config5_full_size(fmt):
+    """BASELINE.json configs[4] (L = 16384) through LEAN by name: 2 MCS against a live oracle run."""
+    cfg = wl.config5()
+    L, r, seed = cfg.L, cfg.rs[0], cfg.seeds[0]
+    use_variant(pgg.VARIANT_LEAN, fmt, L)
+    d = empty_lattice(fmt, L)
+    pgg.pgg_init_lattice(d, fmt, L, cfg.rho0, seed)
+    cnt = torch.zeros(2, dtype=torch.int64, device="cuda")
+    pgg.pgg_sweep(d, fmt, L, r, K, seed, pgg.ORDER_IID, 0, 2, cnt)
+    torch.cuda.synchronize()
+    ref = orc.init(L, cfg.rho0, seed)
+    ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 0, 2, n_threads=orc.max_threads())
+    assert_same(to_host(d, fmt, L), ref, "C5 lattice after 2 MCS")
+    assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)

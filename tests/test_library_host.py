@@ -73,6 +73,15 @@ def test_argument_validation_returns_error_codes():
     assert h.pgg_sweep(fake, 0, 64, 4.0, 0.5, 1, 9, 0, 1, None, None) == pgg.ERR_UNSUPPORTED
     assert h.pgg_sweep(fake, 0, 64, 4.0, 0.5, 1, 0, 2**32 - 1, 2, None, None) == pgg.ERR_BAD_PARAM
     assert h.pgg_density(fake, 0, 64, None, None) == pgg.ERR_NULL
+    # one rule for the upper end (include/pgg.h): site indices are uint32, so L <= 65532 everywhere
+    cnt = C.c_uint64(0)
+    for L_bad in (65536, 65540):
+        assert h.pgg_init_lattice(fake, 0, L_bad, 0.5, 1, None) == pgg.ERR_BAD_L
+        assert h.pgg_sweep(fake, 0, L_bad, 4.0, 0.5, 1, 0, 0, 1, None, None) == pgg.ERR_BAD_L
+        assert h.pgg_density(fake, 0, L_bad, C.byref(cnt), None) == pgg.ERR_BAD_L
+        assert not pgg.pgg_variant_supported(pgg.VARIANT_V0, pgg.FMT_U8, L_bad)
+    assert h.pgg_probe_draw_rate(0, 1, C.byref(cnt), None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_probe_draw_rate(4, 1, None, None) == pgg.ERR_NULL
     # the paper's double-tiling schedule needs L % 8 == 0 and has no phase classes
     assert h.pgg_sweep(fake, 0, 12, 4.0, 0.5, 1, pgg.ORDER_DTILE, 0, 1, None, None) == pgg.ERR_BAD_L
     assert h.pgg_sweep(fake, 0, 64, 4.0, 0.0, 1, pgg.ORDER_DTILE, 0, 1, None, None) == pgg.ERR_BAD_PARAM

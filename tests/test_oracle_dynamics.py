@@ -289,10 +289,65 @@ def test_pack_unpack_bits_layout():
 
 
 def test_rs_sweep_counts_and_site_coverage():
-    """D8: random sequential: counts are recounts; an MCS visits ~ (1 - 1/e) of the sites."""
+    """D8: random sequential: counts are recounts; one MCS is L^2 picks of a uniformly drawn focal
+    site, so a given site is never picked with probability (1 - 1/N)^N ~ 1/e.
+    Observable through the dynamics: at r = 4, K = 1e-3 a lone cooperator in a defector sea
+    (payoff r - 5 = -1 against its neighbours' 2r/5 = 1.6) turns defector the first
+    time it is the focal site, whatever direction it draws, and no defector ever adopts from it.
+    So the lone cooperators that survive one MCS are exactly the never-picked ones."""
     L = 32
     lat = orc.init(L, 0.5, 2)
     before = lat.copy()
     counts = orc.rs_sweep(lat, 4.0, 0.5, 2, 0, 3)
     assert int(counts[-1]) == int(lat.sum())
     assert np.any(lat != before)
+    L, spacing = 200, 5
+    survivors, n_lone = 0, 0
+    for seed in (3, 4, 5):
+        lat = np.zeros((L, L), dtype=np.uint8)
+        lat[2::spacing, 2::spacing] = 1          # isolated: 5 apart, neighbourhoods do not touch
+        lone = lat.copy()
+        n_lone += int(lone.sum())
+        c = orc.rs_sweep(lat, 4.0, 1e-3, seed, 0, 1)
+        assert not np.any(lat & (1 - lone)), "a defector adopted cooperation from a poorer neighbour"
+        assert int(c[0]) == int(lat.sum())
+        survivors += int(lat.sum())
+    p = (1.0 - 1.0 / (L * L)) ** (L * L)         # = 0.36787..., 1/e to four digits
+    sigma = (n_lone * p * (1 - p)) ** 0.5
+    assert abs(survivors - n_lone * p) < 4 * sigma, (survivors, n_lone * p, sigma)
+    assert abs(1 - survivors / n_lone - (1 - np.exp(-1))) < 0.03   # visited fraction ~ 1 - 1/e
+
+
+def test_step_accepts_strictly_below_the_threshold_in_every_direction():
+    """D3 / D6: x adopts s_y iff u < T (strict), with y the neighbour in direction
+    0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1).  T comes from orc_flip_threshold, whose direction
+    table the 4x4 brute force pins; s_y is read here by numpy indexing, so the separate
+    direction table inside orc_step_given_draw is checked against both.  P(u < T) = T / 2^32
+    is Eq. (3) only with the strict compare: `<=` would pass every other pin."""
+    di, dj = (-1, 1, 0, 0), (0, 0, -1, 1)
+    table = orc.accept_table(3.9, 0.5)
+    rng = np.random.default_rng(12)
+    n_checked = 0
+    for L, p in ((8, 0.5), (12, 0.3), (4, 0.5)):
+        for rep in range(6):
+            lat = wl.random_lattice(L, p, seed=100 * L + rep)
+            for _ in range(40):
+                i, j = (int(v) for v in rng.integers(0, L, size=2))
+                for d in range(4):
+                    sx = int(lat[i, j])
+                    sy = int(lat[(i + di[d]) % L, (j + dj[d]) % L])
+                    T = orc.flip_threshold(lat, table, i, j, d)
+                    if sx == sy:
+                        assert T == 0
+                        for u in (0, 1, 0x7FFFFFFF, 0xFFFFFFFF):
+                            assert orc.step_given_draw(lat, table, i, j, d, u) == sx
+                        continue
+                    assert T == int(table[orc.table_index(orc.A(lat, i, j) - orc.A(lat, (i + di[d]) % L, (j + dj[d]) % L),
+                                                          sx - sy)])
+                    if T > 0:
+                        assert orc.step_given_draw(lat, table, i, j, d, T - 1) == sy, "u = T - 1 must be accepted"
+                        assert orc.step_given_draw(lat, table, i, j, d, 0) == sy
+                    assert orc.step_given_draw(lat, table, i, j, d, T) == sx, "u = T must be rejected (strict <)"
+                    assert orc.step_given_draw(lat, table, i, j, d, 0xFFFFFFFF) == sx
+                    n_checked += 1
+    assert n_checked > 500
