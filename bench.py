@@ -88,11 +88,12 @@ class ClockSampler:
 ORC_ORDER = 0  # oracle order mode of the cpu_baseline / reference legs (set from --order)
 
 
-def oracle_sample(L: int, max_mcs: int, min_seconds: float):
-    """Time the oracle (as it stands) on `max_mcs` MCS of the workload, all host threads."""
+def oracle_sample(L: int, max_mcs: int, min_seconds: float, threads: int = 0):
+    """Time the oracle (as it stands) on the first MCS of the workload (MCS 0 .. done-1 from the
+    Bernoulli start), on `threads` host threads (0 = all)."""
     import numpy as np
     import oracle as orc
-    threads = orc.max_threads()
+    threads = threads or orc.max_threads()
     lat = orc.init(L, RHO0, SEED)
     done, t0 = 0, time.perf_counter()
     while done < max_mcs:
@@ -136,8 +137,9 @@ def run_reference(args):
         orc.sweep(lat, R, K_NOISE, SEED, ORC_ORDER, t, 1, n_threads=threads); t += 1
     dt = time.perf_counter() - t0
     value = args.steps * L * L / dt
-    sample = (f"each step = 1 MCS (MCS {args.warmup}..{t - 1}) of the L={L} workload from the "
-              f"Bernoulli(0.5) seed-1 start; oracle/pgg_oracle.c -O2, rows of a class split over threads")
+    sample = (f"each step = 1 MCS; timed window = MCS {args.warmup}..{t - 1} of the L={L} workload from the "
+              f"Bernoulli(0.5) seed-1 start (after {args.warmup} warm-up MCS the state is sparser than at MCS 0, so the "
+              f"rate differs from cpu_baseline's window MCS 0..7); oracle/pgg_oracle.c -O2, rows of a class split over threads")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "updates/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
@@ -275,6 +277,21 @@ def run_ours(args):
     p1.record(stream)
     stream.synchronize()
     draws_per_s = n_draws / (p0.elapsed_time(p1) * 1e-3)
+    # the draw fraction of the workload: sites with a neighbour of the other strategy (S9), sampled
+    # at log-spaced MCS of the same deterministic run (untimed) and averaged over time
+    d_if = torch.zeros(1, dtype=torch.int64, device="cuda")
+    stops = sorted({0, n_mcs} | {min(n_mcs, int(round(10 ** (a / 4.0)))) for a in range(0, 4 * 8)})
+    pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
+    f_t, t_prev = [], 0
+    for t_stop in stops:
+        if t_stop > t_prev:
+            pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, t_prev, t_stop - t_prev, None, stream)
+            t_prev = t_stop
+        pgg.pgg_count_interface(d_lat, fmt, L, d_if, stream)
+        stream.synchronize()
+        f_t.append((t_stop, d_if.item() / float(L * L)))
+    draw_fraction = (sum(0.5 * (f_t[a][1] + f_t[a + 1][1]) * (f_t[a + 1][0] - f_t[a][0]) for a in range(len(f_t) - 1))
+                     / max(1, n_mcs)) if n_mcs else f_t[0][1]
 
     # ---- roofline of the dominant kernel (the phase kernel; 16 launches per MCS)
     peak, peak_src = load_peaks()
@@ -301,6 +318,21 @@ def run_ours(args):
                 f"{args.fmt}_L{L}_bytes_per_launch" + ("_dtile" if dtile else ""))
         except (ValueError, OSError):
             pass
+    # the ALU view: STEP draws per second against the Philox-only ceiling
+    sweep_rate = args.steps * updates_per_step / (sweep_ms * 1e-3)
+    alu = {"bound": "alu", "achieved": sweep_rate * draw_fraction / 1e9, "peak": draws_per_s / 1e9,
+           "unit": "Gdraw/s", "frac": sweep_rate * draw_fraction / draws_per_s,
+           "draw_fraction": draw_fraction,
+           "note": "achieved = updates/s x the time-averaged fraction of sites that need a draw "
+                   "(pgg_count_interface at log-spaced MCS of the same run); peak = pgg_probe_draw_rate, "
+                   "a kernel that makes STEP draws only (DESIGN.md section 5)"}
+    if fmt == pgg.FMT_BITS and not dtile:
+        # the packed lattice is L2-resident: its bound is the integer pipes, not HBM
+        alu.update({"traffic": roofline["traffic"], "kernel": roofline["kernel"], "avg_launch_us": phase_us,
+                    "hbm_context": {k: roofline[k] for k in ("achieved", "peak", "frac", "algorithmic_bytes_per_launch")}})
+        roofline = alu
+    else:
+        roofline["alu_context"] = {k: alu[k] for k in ("achieved", "peak", "unit", "frac", "draw_fraction")}
 
     out = {
         "metric": METRIC, "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps,
@@ -330,10 +362,13 @@ def run_ours(args):
     }
     if world == 1 and not args.no_cpu_baseline:
         v, threads, n_done, dt = oracle_sample(L, max_mcs=8, min_seconds=10.0)
+        v1, _, n1, dt1 = oracle_sample(L, max_mcs=1, min_seconds=0.0, threads=1)
         out["cpu_baseline"] = {"value": v, "unit": "updates/s", "cores": threads, "kind": "oracle",
-                               "sample": f"first {n_done} MCS of the same L={L} workload ({dt:.1f} s wall), "
-                                         f"oracle/pgg_oracle.c as it stands, class rows split over "
-                                         f"{threads} OpenMP threads"}
+                               "sample": f"MCS 0..{n_done - 1} (the dense start: rho_C 0.5 -> 0.04) of the same L={L} "
+                                         f"workload ({dt:.1f} s wall), oracle/pgg_oracle.c as it stands, class rows "
+                                         f"split over {threads} OpenMP threads",
+                               "one_thread": {"value": v1, "unit": "updates/s", "cores": 1,
+                                              "sample": f"MCS 0 of the same workload ({dt1:.1f} s wall)"}}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -75,9 +75,10 @@ enum { PGG_FMT_U8 = 0, PGG_FMT_BITS = 1 };
 enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
 
 /* Kernel variants of the phase step (all bit-identical).
- * PGG_VARIANT_AUTO picks by measurement (profiles/r1_ring_design_notes.md):
- * RESIDENT for L <= 320 or many lattices (B L^2 >= 16 * 512^2, L <= 512); RING
- * (uint8) / BAND (bit-packed) for L >= 2048 and for uint8 L = 512, 1024; else V0. */
+ * PGG_VARIANT_AUTO picks by measurement (profiles/r2_auto_small_lattices.md, profiles/r2_lean_notes.md):
+ * RESIDENT for L <= 320, and for L <= 512 from 3 lattices (6 at L = 512; uint8 L = 512: from 20, RING
+ * below that); LEAN for the bit-packed layout at L = 1024 .. 32768 (powers of two); RING (uint8) / BAND
+ * (bit-packed) for the other L >= 2048 and for uint8 L = 512, 1024; else V0.                          */
 enum {
     PGG_VARIANT_AUTO = 0,
     PGG_VARIANT_V0 = 1,   /* one thread per active site, global loads, any L % 4 == 0 */
@@ -167,6 +168,13 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L);
  * before return) = draws the launch makes; the caller times the launch with events on `stream`.
  * No lattice is touched.  Errors: PGG_ERR_NULL, PGG_ERR_BAD_PARAM (iters == 0), PGG_ERR_CUDA. */
 int32_t pgg_probe_draw_rate(uint32_t iters, uint64_t seed, uint64_t* h_n_draws, void* stream);
+
+/* Number of sites with at least one nearest neighbour of the other strategy: the sites for which
+ * an elementary step needs its random draw (S9: for all others no draw can change
+ * the state).  count / L^2 is the draw fraction of the state, the factor between the Philox-only
+ * ceiling (pgg_probe_draw_rate) and the update rate it allows.  d_count: device uint64, overwritten.
+ * Errors as pgg_density.                                                                      */
+int32_t pgg_count_interface(const void* d_lat, int32_t fmt, uint32_t L, uint64_t* d_count, void* stream);
 
 /* Number of kernels this library has launched in this process (monotone).       */
 uint64_t pgg_launch_count(void);

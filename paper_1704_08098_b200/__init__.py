@@ -42,6 +42,7 @@ SIGNATURES = {
     "pgg_get_variant_used": (C.c_int32, []),
     "pgg_variant_supported": (C.c_int32, [C.c_int32, C.c_int32, C.c_uint32]),
     "pgg_probe_draw_rate": (C.c_int32, [C.c_uint32, C.c_uint64, _u64p, C.c_void_p]),
+    "pgg_count_interface": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_void_p, C.c_void_p]),
     "pgg_launch_count": (C.c_uint64, []),
     "pgg_last_error": (C.c_char_p, []),
 }
@@ -139,6 +140,10 @@ def pgg_probe_draw_rate(iters: int, seed: int = 1, stream=None) -> int:
     n = C.c_uint64(0)
     _check(lib().pgg_probe_draw_rate(iters, seed, C.byref(n), _stream(stream)))
     return int(n.value)
+
+
+def pgg_count_interface(d_lat, fmt: int, L: int, d_count, stream=None) -> None:
+    _check(lib().pgg_count_interface(_ptr(d_lat), fmt, L, _ptr(d_count), _stream(stream)))
 
 
 def pgg_launch_count() -> int:

@@ -153,10 +153,14 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     // of the streaming kernels uint8 is fastest on RING, bit-packed on BAND
     const bool res_ok = pgg::resident_supported(fmt, L);
     if (variant == PGG_VARIANT_AUTO) {
-        // RESIDENT takes one SM per lattice whatever B is, and its time grows with L^2 (1.5 us per
-        // phase at L = 64, 7-13 at L = 512); a per-phase launch costs 4-5 us until B L^2 makes it
-        // throughput-bound (L = 512: V0 6 us at B = 8, 24 at B = 64).  So: small lattices, or many.
-        const bool res_pays = L <= 320 || (unsigned long long)B * L * L >= 16ull * 512ull * 512ull;
+        // Measured rule (profiles/r2_auto_small_lattices.md, us per phase at r = 3.8).  RESIDENT takes one SM
+        // per lattice whatever B is and grows with L^2 (1.5 us at L = 128, 2.8 at 320, 4.7 at 400, 6.9 at
+        // 512); a V0 launch costs 4.2 us until B L^2 makes it throughput-bound.  So RESIDENT for L <= 320,
+        // and above that from the batch size at which V0 has become slower: 3 lattices (L <= 448), 6 (L = 512).
+        // uint8 L = 512 is also a whole-row strip for RING (4.2 us at B = 1, 6.8 at 13, 9.2 at 52): RING below
+        // 20 lattices, RESIDENT from there (config 4).
+        const bool ring_512 = fmt == PGG_FMT_U8 && L == 512 && ring_ok && B < 20;
+        const bool res_pays = L <= 320 || (!ring_512 && B >= (L <= 448 ? 3u : 6u));
         // the streaming kernels need long rows (or whole-row strips: uint8 L = 512 * 2^k) to beat
         // V0's launch-bound 4-5 us; below that their fixed cost is ~9.5 us per launch
         const bool stream_pays = L >= 2048 || (fmt == PGG_FMT_U8 && L >= 512 && (L & (L - 1)) == 0);
@@ -465,6 +469,25 @@ int32_t pgg_probe_draw_rate(uint32_t iters, uint64_t seed, uint64_t* h_n_draws, 
     pgg::draw_ceiling_kernel<<<grid, pgg::kProbeThreads, 0, s>>>(sk, iters, d_sink);
     PGG_LAUNCHED();
     *h_n_draws = 2ull * iters * grid * pgg::kProbeThreads;
+    return PGG_OK;
+}
+
+int32_t pgg_count_interface(const void* d_lat, int32_t fmt, uint32_t L, uint64_t* d_count, void* stream)
+{
+    int32_t rc = check_lattice_args(d_lat, fmt, L);
+    if (rc != PGG_OK) return rc;
+    if (d_count == nullptr) return fail(PGG_ERR_NULL, "d_count is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    PGG_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint64_t), s));
+    const uint32_t n = L * L;
+    const uint32_t grid = std::min<uint32_t>((n + 255u) / 256u, 148u * 32u);
+    if (fmt == PGG_FMT_U8)
+        pgg::interface_count_kernel<pgg::kFmtU8><<<grid, 256, 0, s>>>(static_cast<const uint8_t*>(d_lat), L,
+                                                                    reinterpret_cast<unsigned long long*>(d_count));
+    else
+        pgg::interface_count_kernel<pgg::kFmtBits><<<grid, 256, 0, s>>>(static_cast<const uint8_t*>(d_lat), L,
+                                                                      reinterpret_cast<unsigned long long*>(d_count));
+    PGG_LAUNCHED();
     return PGG_OK;
 }
 

@@ -2,7 +2,7 @@
 
     python -m paper_1704_08098_b200.physics stationary [--L 400] [--mcs 20000] [--seeds 101 102 103 104]
                                                        [--order iid|perm] [--rs 3.6 3.65 ...]
-    python -m paper_1704_08098_b200.physics decay --r 3.7443 [--L 2048] [--mcs 100000] [--seeds 1..16]
+    python -m paper_1704_08098_b200.physics decay --r 3.7443 [--L 2048] [--mcs 100000] [--seeds 1..16] [--fmt bits]
     python -m paper_1704_08098_b200.physics fig5 [--order dtile|iid] [--mcs 2000]
 
 ``stationary``: rho_C(r) of BASELINE.json configs[1] -- the time average of Eq. (4) over
@@ -23,7 +23,7 @@ import math
 
 import numpy as np
 
-from . import (FMT_U8, ORDER_DTILE, ORDER_IID, ORDER_PERM, pgg_init_lattice, pgg_run_ensemble, pgg_sweep)
+from . import (FMT_BITS, FMT_U8, ORDER_DTILE, ORDER_IID, ORDER_PERM, pgg_init_lattice, pgg_run_ensemble, pgg_sweep)
 
 
 def run_traces(L, rs, seeds, K, rho0, n_mcs, order=ORDER_IID, fmt=FMT_U8, chunk=None):
@@ -68,10 +68,10 @@ def log_times(n_mcs, per_decade=8):
     return sorted(ts)
 
 
-def decay(r, seeds, L=2048, n_mcs=100000, K=0.5, rho0=0.5, order=ORDER_IID):
+def decay(r, seeds, L=2048, n_mcs=100000, K=0.5, rho0=0.5, order=ORDER_IID, fmt=FMT_U8):
     """-> list of rows {t, rho, rho_err, delta_eff, delta_err}: seed average of rho_C(t), error from the
     scatter between seeds; delta_eff(t) between t/8 and t with a seed-jackknife error."""
-    tr = run_traces(L, [r] * len(seeds), seeds, K, rho0, n_mcs, order).astype(np.float64) / (L * L)
+    tr = run_traces(L, [r] * len(seeds), seeds, K, rho0, n_mcs, order, fmt).astype(np.float64) / (L * L)
     rows = []
     n = len(seeds)
     for t in log_times(n_mcs):
@@ -123,6 +123,7 @@ def main():
     ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"])
     ap.add_argument("--rs", type=float, nargs="+", default=None)
     ap.add_argument("--r", type=float, default=3.7443)
+    ap.add_argument("--fmt", default="u8", choices=["u8", "bits"], help="lattice layout (decay only; same trajectories)")
     args = ap.parse_args()
     order = {"iid": ORDER_IID, "perm": ORDER_PERM, "dtile": ORDER_DTILE}[args.order]
     if args.what == "fig5":
@@ -134,9 +135,11 @@ def main():
         print(json.dumps({"what": "stationary", "order": args.order, "L": args.L or 400, "mcs": args.mcs or 20000,
                           "rows": [{"r": r, **v} for r, v in res.items()]}))
     else:
-        rows = decay(args.r, args.seeds or list(range(1, 17)), args.L or 2048, args.mcs or 100000, order=order)
-        print(json.dumps({"what": "decay", "order": args.order, "r": args.r, "L": args.L or 2048,
-                          "mcs": args.mcs or 100000, "rows": rows}))
+        seeds = args.seeds or list(range(1, 17))
+        rows = decay(args.r, seeds, args.L or 2048, args.mcs or 100000, order=order,
+                     fmt=FMT_BITS if args.fmt == "bits" else FMT_U8)
+        print(json.dumps({"what": "decay", "order": args.order, "r": args.r, "L": args.L or 2048, "fmt": args.fmt,
+                          "mcs": args.mcs or 100000, "seeds": seeds, "rows": rows}))
 
 
 if __name__ == "__main__":

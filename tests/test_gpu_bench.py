@@ -34,8 +34,12 @@ def test_bench_line_has_the_contract_keys():
     assert d["gpu_launches"] == 2 * (1 + 1 + 1 + 16 * 20 + 1)
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    a = r["alu_context"]                                  # the draws against the Philox-only ceiling
+    assert a["unit"] == "Gdraw/s" and 0.0 < a["draw_fraction"] <= 1.0 and 0.0 < a["frac"] < 1.5
+    assert d["ceilings"]["philox_step_draws_per_s"] > 1e10
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == "updates/s"
+    assert c["one_thread"]["cores"] == 1 and c["one_thread"]["value"] > 0 and "MCS 0" in c["sample"]
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
 
 
@@ -56,3 +60,13 @@ def test_bench_line_for_the_papers_schedule():
     r = d["roofline"]
     assert r["algorithmic_bytes_per_launch"] == 1024 * 1024 * 1.25 and "dtile_part_kernel" in r["kernel"]
     assert d["value"] > 0 and d["e2e"]["value"] > 0 and 0.0 <= d["final_rho_C"] <= 1.0
+
+
+def test_bench_line_for_the_bit_packed_layout():
+    """--fmt bits: the packed lattice is L2-resident, so the roofline object is the ALU one (STEP draws per
+    second against the Philox-only ceiling) with the HBM view kept as context."""
+    d = run_bench("--fmt", "bits", "--no-cpu-baseline")
+    r = d["roofline"]
+    assert d["dtype"].startswith("u1") and d["config"]["variant"] == 11      # AUTO -> LEAN
+    assert r["bound"] == "alu" and r["unit"] == "Gdraw/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert 0.0 < r["draw_fraction"] <= 1.0 and r["hbm_context"]["algorithmic_bytes_per_launch"] == 1024 * 1024 * 17 / 16 / 8

@@ -115,6 +115,23 @@ def test_density_parity(fmt):
         assert int(out.item()) == orc.count(lat) == int(lat.sum())
 
 
+@pytest.mark.parametrize("fmt", FMTS)
+def test_interface_count(fmt):
+    """pgg_count_interface = sites with a nearest neighbour of the other strategy (the sites an
+    elementary step needs its draw for, S9); numpy rolls are the plain definition."""
+    for L, p in ((64, 0.5), (416, 0.3), (32, 0.0), (1024, 0.05)):
+        lat = wl.random_lattice(L, p, seed=3 * L)
+        want = 0
+        diff = np.zeros_like(lat, dtype=bool)
+        for ax, sh in ((0, 1), (0, -1), (1, 1), (1, -1)):
+            diff |= np.roll(lat, sh, axis=ax) != lat
+        want = int(diff.sum())
+        out = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+        pgg.pgg_count_interface(to_device(lat, fmt), fmt, L, out)
+        torch.cuda.synchronize()
+        assert int(out.item()) == want
+
+
 # ---------------------------------------------------------------- config 1 in full
 @pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("fmt", FMTS)

@@ -78,3 +78,33 @@ def test_perm_order_is_biased(gpu_tables):
     ref = rs_table()
     for r in (3.8, 3.9, 4.0):
         assert n_sigma(perm[r], ref[r]) > 10.0
+
+
+def test_critical_decay_brackets_the_threshold():
+    """BASELINE.json configs[2] at its size and length (L = 2048, 16 seeds, 10^5 MCS; bit-packed, so the
+    run takes about a minute): on either side of the threshold r_c = 3.7445(1) (DESIGN.md section 7;
+    the paper: 3.7443(4)) the local decay exponent delta_eff(t) = -ln[rho(t)/rho(t/8)]/ln 8
+    bends the way directed percolation says it must: below r_c it keeps growing past the
+    DP value 0.4505 (the density dies exponentially), above r_c it falls back towards 0 (the density
+    saturates).  The decay from a random start is not a clean power law before t ~ 10^4 (S20), so only the
+    last decade is used."""
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    seeds = list(range(1, 17))
+
+    def d_eff(r):
+        rows = {q["t"]: q for q in physics.decay(r, seeds, L=2048, n_mcs=100000, fmt=pgg.FMT_BITS)}
+        ts = sorted(rows)
+        late = [rows[t] for t in ts if t >= 30000 and "delta_eff" in rows[t]]
+        return rows, late
+
+    sub_rows, sub = d_eff(3.7440)
+    sup_rows, sup = d_eff(3.7450)
+    # sub-critical: delta_eff passes the DP value and keeps rising (or the seeds die out altogether)
+    dead = sub_rows[100000]["alive"] == 0
+    assert dead or sub[-1]["delta_eff"] > 0.4505 + 3 * sub[-1]["delta_err"], sub[-1]
+    assert dead or sub[-1]["delta_eff"] > sub[0]["delta_eff"]
+    # super-critical: every seed alive, delta_eff stays below the DP value and has stopped growing
+    assert sup_rows[100000]["alive"] == len(seeds)
+    assert sup[-1]["delta_eff"] < 0.4505 - 3 * sup[-1]["delta_err"], sup[-1]
+    assert sup[-1]["delta_eff"] < max(q["delta_eff"] for q in sup) + 1e-12
+    assert sup_rows[100000]["rho"] > 2 * sub_rows[100000]["rho"]
