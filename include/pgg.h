@@ -28,8 +28,11 @@
  * Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller
  * owns every buffer.  `stream` is a cudaStream_t passed as void* (NULL = the
  * legacy default stream).  All device work is enqueued on `stream`; no entry
- * point synchronises with the host, results are valid once the caller has
- * synchronised the stream.  Temporary device memory is taken and returned
+ * point waits for the stream or the device (pgg_phase_classes, which returns host data, is the one
+ * exception and says so): per-lattice parameters reach the device as kernel arguments, not by
+ * copies from pageable memory, so host arrays may be freed on return.  Results are valid once
+ * the caller has synchronised the stream.  The kernel-variant switch (pgg_set_variant) and the
+ * environment knobs DESIGN.md lists are process-wide; a call uses the current CUDA device.  Temporary device memory is taken and returned
  * with the stream-ordered allocator (cudaMallocAsync / cudaFreeAsync).
  */
 #ifndef PGG_H_
@@ -83,7 +86,7 @@ enum {
     PGG_VARIANT_AUTO = 0,
     PGG_VARIANT_V0 = 1,   /* one thread per active site, global loads, any L % 4 == 0 */
     PGG_VARIANT_TILE = 2, /* smem tile + 3-site halo, bulk-async staged, compaction   */
-    PGG_VARIANT_FUSED = 3,/* several phases per tile residency (temporal blocking)    */
+    /* 3 is unused (a temporal-blocking variant was never built: DESIGN.md section 9)   */
     PGG_VARIANT_PIPE = 4, /* TILE staging as a producer/consumer warp pipeline        */
     PGG_VARIANT_BAND = 5, /* row bands of wide strips streamed through a smem ring    */
     PGG_VARIANT_RING = 6, /* BAND's data movement, consumer cut to the fewest instr.  */

@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "pgg_oracle.c"
+_SRC_PD = _HERE / "pd_oracle.c"   # the prisoner's dilemma, same library
 _LIB = _HERE / "liboracle_pgg.so"
 
 ORDER_IID = 0
@@ -26,10 +27,10 @@ ORDER_DTILE = 2  # the paper's double-tiling schedule
 
 def build(force: bool = False) -> Path:
     """Compile the oracle with gcc (-O2, OpenMP for the optional row split)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < max(_SRC.stat().st_mtime, _SRC_PD.stat().st_mtime):
         tmp = _LIB.with_suffix(f".{os.getpid()}.tmp.so")
         cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-               "-o", str(tmp), str(_SRC), "-lm"]
+               "-o", str(tmp), str(_SRC), str(_SRC_PD), "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)
     return _LIB
@@ -96,6 +97,25 @@ def lib() -> C.CDLL:
         L.orc_unpack_bits.restype = None
         L.orc_max_threads.argtypes = []
         L.orc_max_threads.restype = C.c_int
+        d4 = [C.c_double] * 4
+        L.orc_pd_payoff_literal.argtypes = [u8p, C.c_int, C.c_int, C.c_int] + d4
+        L.orc_pd_payoff_literal.restype = C.c_double
+        L.orc_pd_nc.argtypes = [u8p, C.c_int, C.c_int, C.c_int]
+        L.orc_pd_nc.restype = C.c_int
+        L.orc_pd_payoff.argtypes = [C.c_int, C.c_int] + d4
+        L.orc_pd_payoff.restype = C.c_double
+        L.orc_pd_table_index.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.orc_pd_table_index.restype = C.c_int
+        L.orc_pd_accept_table.argtypes = d4 + [C.c_double, u32p]
+        L.orc_pd_accept_table.restype = None
+        L.orc_pd_flip_threshold.argtypes = [u8p, C.c_int, u32p, C.c_int, C.c_int, C.c_int]
+        L.orc_pd_flip_threshold.restype = C.c_uint32
+        L.orc_pd_step_given_draw.argtypes = [u8p, C.c_int, u32p, C.c_int, C.c_int, C.c_int, C.c_uint32]
+        L.orc_pd_step_given_draw.restype = C.c_int
+        L.orc_pd_phase.argtypes = [u8p, C.c_int, u32p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int]
+        L.orc_pd_phase.restype = C.c_int64
+        L.orc_pd_sweep.argtypes = [u8p, C.c_int] + d4 + [C.c_double, C.c_uint64, C.c_int, C.c_uint32, C.c_uint32, u64p]
+        L.orc_pd_sweep.restype = C.c_int
         _lib = L
     return _lib
 
@@ -274,3 +294,56 @@ def unpack_bits(words, L) -> np.ndarray:
 
 def max_threads() -> int:
     return lib().orc_max_threads()
+
+
+# ---------------------------------------------------------------- prisoner's dilemma (pd_oracle.c)
+def pd_payoff_literal(lat, i, j, R, S, T, P) -> float:
+    lat = _lat(lat)
+    return float(lib().orc_pd_payoff_literal(_u8(lat), lat.shape[0], i, j, R, S, T, P))
+
+
+def pd_nc(lat, i, j) -> int:
+    lat = _lat(lat)
+    return lib().orc_pd_nc(_u8(lat), lat.shape[0], i, j)
+
+
+def pd_payoff(s, n, R, S, T, P) -> float:
+    return float(lib().orc_pd_payoff(s, n, R, S, T, P))
+
+
+def pd_table_index(sx, nx, ny) -> int:
+    return lib().orc_pd_table_index(sx, nx, ny)
+
+
+def pd_accept_table(R, S, T, P, K) -> np.ndarray:
+    out = np.zeros(50, dtype=np.uint32)
+    lib().orc_pd_accept_table(R, S, T, P, K, _u32(out))
+    return out
+
+
+def pd_flip_threshold(lat, table, i, j, direction) -> int:
+    lat = _lat(lat)
+    table = np.ascontiguousarray(table, dtype=np.uint32)
+    return int(lib().orc_pd_flip_threshold(_u8(lat), lat.shape[0], _u32(table), i, j, direction))
+
+
+def pd_step_given_draw(lat, table, i, j, direction, u) -> int:
+    lat = _lat(lat)
+    table = np.ascontiguousarray(table, dtype=np.uint32)
+    return lib().orc_pd_step_given_draw(_u8(lat), lat.shape[0], _u32(table), i, j, direction, u)
+
+
+def pd_phase(lat, table, seed, t, k, c, visit=0) -> int:
+    assert lat.dtype == np.uint8 and lat.flags.c_contiguous
+    table = np.ascontiguousarray(table, dtype=np.uint32)
+    return int(lib().orc_pd_phase(_u8(lat), lat.shape[0], _u32(table), seed, t, k, c, visit))
+
+
+def pd_sweep(lat, R, S, T, P, K, seed, order_mode=ORDER_IID, t_begin=0, n_mcs=1):
+    """In-place prisoner's-dilemma sweep under the 16-sublattice schedule; returns counts[n_mcs]."""
+    assert lat.dtype == np.uint8 and lat.flags.c_contiguous
+    counts = np.zeros(max(n_mcs, 1), dtype=np.uint64)
+    rc = lib().orc_pd_sweep(_u8(lat), lat.shape[0], R, S, T, P, K, seed, order_mode, t_begin, n_mcs, _u64(counts))
+    if rc != 0:
+        raise ValueError("orc_pd_sweep: bad arguments")
+    return counts[:n_mcs]

@@ -21,7 +21,8 @@ OK = 0
 ERR_NULL, ERR_BAD_L, ERR_BAD_PARAM, ERR_ALIGN, ERR_UNSUPPORTED, ERR_CUDA = -1, -2, -3, -4, -5, -6
 FMT_U8, FMT_BITS = 0, 1
 ORDER_IID, ORDER_PERM, ORDER_DTILE = 0, 1, 2
-VARIANT_AUTO, VARIANT_V0, VARIANT_TILE, VARIANT_FUSED, VARIANT_PIPE, VARIANT_BAND, VARIANT_RING, VARIANT_SPLIT, VARIANT_DYN, VARIANT_RESIDENT = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
+VARIANT_AUTO, VARIANT_V0, VARIANT_TILE = 0, 1, 2
+VARIANT_PIPE, VARIANT_BAND, VARIANT_RING, VARIANT_SPLIT, VARIANT_DYN, VARIANT_RESIDENT = 4, 5, 6, 7, 8, 9
 VARIANT_DTILE, VARIANT_LEAN = 10, 11
 
 # name -> (restype, argtypes); also the list of symbols include/pgg.h declares

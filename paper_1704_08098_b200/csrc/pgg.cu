@@ -94,6 +94,23 @@ struct Scratch {
     }
 };
 
+// seeds (and, if h_tables != nullptr, acceptance tables) of B lattices -> device arrays, as kernel arguments
+int32_t upload_params(uint32_t B, const uint64_t* h_seeds, const uint32_t* h_tables, uint64_t* d_seeds,
+                      uint32_t* d_tables, cudaStream_t stream)
+{
+    for (uint32_t first = 0; first < B; first += pgg::kParamPackLattices) {
+        pgg::ParamPack p;
+        p.n = std::min<uint32_t>(pgg::kParamPackLattices, B - first);
+        p.with_tables = h_tables != nullptr ? 1u : 0u;
+        for (uint32_t a = 0; a < p.n; ++a) p.seeds[a] = h_seeds[first + a];
+        if (h_tables != nullptr)
+            std::memcpy(p.tables, h_tables + (size_t)first * pgg::kTableSize, sizeof(uint32_t) * p.n * pgg::kTableSize);
+        pgg::upload_params_kernel<<<1, 256, 0, stream>>>(p, first, d_seeds, d_tables);
+        PGG_LAUNCHED();
+    }
+    return PGG_OK;
+}
+
 int32_t launch_init(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, double rho0,
                     const uint64_t* d_seeds, cudaStream_t stream)
 {
@@ -180,9 +197,8 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
         (variant == PGG_VARIANT_SPLIT && !split_ok) || (variant == PGG_VARIANT_DYN && !pgg::dyn_supported(fmt, L)))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
-    if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_FUSED || variant == PGG_VARIANT_PIPE) && !tile_ok)
+    if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_PIPE) && !tile_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
-    if (variant == PGG_VARIANT_FUSED) return fail(PGG_ERR_UNSUPPORTED, "fused variant not built");
     g_variant_used = variant;
 
     Scratch tmp(stream);
@@ -196,11 +212,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     uint32_t* d_tables = nullptr;
     PGG_CUDA(tmp.alloc((void**)&d_seeds, sizeof(uint64_t) * B));
     PGG_CUDA(tmp.alloc((void**)&d_tables, sizeof(uint32_t) * h_tables.size()));
-    // pageable sources: the runtime stages them before returning, so the host
-    // vectors may die at scope exit
-    PGG_CUDA(cudaMemcpyAsync(d_seeds, h_seeds, sizeof(uint64_t) * B, cudaMemcpyHostToDevice, stream));
-    PGG_CUDA(cudaMemcpyAsync(d_tables, h_tables.data(), sizeof(uint32_t) * h_tables.size(),
-                             cudaMemcpyHostToDevice, stream));
+    {   // as kernel arguments: nothing is copied from pageable memory, the host vectors may die at scope exit
+        int32_t rc = upload_params(B, h_seeds, h_tables.data(), d_seeds, d_tables, stream);
+        if (rc != PGG_OK) return rc;
+    }
 
     if (rho0 >= 0.0) {
         int32_t rc = launch_init(d_lats, fmt, B, L, rho0, d_seeds, stream);
@@ -372,7 +387,8 @@ int32_t pgg_init_lattice(void* d_lat, int32_t fmt, uint32_t L, double rho0, uint
     Scratch tmp(s);
     uint64_t* d_seed = nullptr;
     PGG_CUDA(tmp.alloc((void**)&d_seed, sizeof(uint64_t)));
-    PGG_CUDA(cudaMemcpyAsync(d_seed, &seed, sizeof seed, cudaMemcpyHostToDevice, s));
+    rc = upload_params(1, &seed, nullptr, d_seed, nullptr, s);
+    if (rc != PGG_OK) return rc;
     return launch_init(static_cast<uint8_t*>(d_lat), fmt, 1, L, rho0, d_seed, s);
 }
 
@@ -420,7 +436,10 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
     uint8_t* d_order = nullptr;
     PGG_CUDA(tmp.alloc((void**)&d_seed, sizeof(uint64_t)));
     PGG_CUDA(tmp.alloc((void**)&d_order, 16));
-    PGG_CUDA(cudaMemcpyAsync(d_seed, &seed, sizeof seed, cudaMemcpyHostToDevice, s));
+    {
+        int32_t rc = upload_params(1, &seed, nullptr, d_seed, nullptr, s);
+        if (rc != PGG_OK) return rc;
+    }
     pgg::order_kernel<<<1, 128, 0, s>>>(d_seed, 1, t, 1, 1, order_mode, d_order);
     PGG_LAUNCHED();
     PGG_CUDA(cudaMemcpyAsync(h_out16, d_order, 16, cudaMemcpyDeviceToHost, s));
@@ -430,7 +449,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_LEAN || variant == PGG_VARIANT_DTILE)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_LEAN || variant == PGG_VARIANT_DTILE || variant == 3)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;

@@ -425,8 +425,8 @@ inline bool band_supported(int fmt, uint32_t L)
 
 inline int band_plan(int fmt, uint32_t L, uint32_t B, BandPlan* p)
 {
-    static int sm_count = 0, smem_optin = 0;
-    if (sm_count == 0) {
+    int sm_count = 0, smem_optin = 0;  // per call: the function attribute is per device, and a plan costs nothing next to 16 n_mcs launches
+    {
         int dev = 0, sms = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;

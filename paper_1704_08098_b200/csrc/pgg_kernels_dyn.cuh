@@ -286,8 +286,8 @@ inline bool dyn_supported(int fmt, uint32_t L)
 template <int NW>
 inline int dyn_plan_nw(uint32_t L, uint32_t B, RingPlan* p)
 {
-    static int smem_optin = 0;
-    if (smem_optin == 0) {
+    int smem_optin = 0;  // per call (the function attribute is per device)
+    {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;

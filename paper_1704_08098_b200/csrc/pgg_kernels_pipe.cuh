@@ -255,8 +255,8 @@ phase_pipe_kernel(PhaseArgs a, uint32_t m, uint32_t k, TilePlan g)
 // ---------------------------------------------------------------------------
 inline int pipe_plan(int fmt, uint32_t L, uint32_t B, TilePlan* p)
 {
-    static int sm_count = 0, smem_optin = 0;
-    if (sm_count == 0) {
+    int sm_count = 0, smem_optin = 0;  // per call: the function attribute is per device, and a plan costs nothing next to 16 n_mcs launches
+    {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;

@@ -221,7 +221,7 @@ sweep_resident_kernel(PhaseArgs a, uint32_t m0, uint32_t n_chunk, ResPlan g)
 
 inline int resident_plan(int fmt, uint32_t L, ResPlan* p)
 {
-    static bool attr_set = false;
+    bool attr_set = false;  // per call (the function attribute is per device)
     p->PW = (L + 6 + 31) / 32;
     p->n_words = (L + 6) * p->PW;
     p->list_cap = (L / 4) * (L / 4);

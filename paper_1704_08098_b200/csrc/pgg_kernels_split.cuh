@@ -311,8 +311,8 @@ inline bool split_supported(int fmt, uint32_t L)
 
 inline int split_plan(uint32_t L, uint32_t B, RingPlan* p)
 {
-    static int smem_optin = 0;
-    if (smem_optin == 0) {
+    int smem_optin = 0;  // per call (the function attribute is per device)
+    {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;

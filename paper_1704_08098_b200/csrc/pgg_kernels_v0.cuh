@@ -8,6 +8,30 @@
 namespace pgg {
 
 // ---------------------------------------------------------------------------
+// Per-lattice parameters (seed, acceptance table) travel to the device as KERNEL ARGUMENTS of
+// this little kernel, five lattices per launch: no copy from pageable host memory, so no entry
+// point ever waits for the stream, the caller's host arrays may die on return, and the calls can
+// be captured into a CUDA graph.
+// ---------------------------------------------------------------------------
+constexpr int kParamPackLattices = 5;  // 5 x (8 + 612) bytes + header < the 4 KB argument limit
+struct ParamPack {
+    uint32_t n;                                     // lattices in this pack
+    uint32_t with_tables;
+    uint64_t seeds[kParamPackLattices];
+    uint32_t tables[kParamPackLattices * kTableSize];
+};
+
+__global__ void __launch_bounds__(256)
+upload_params_kernel(const __grid_constant__ ParamPack p, uint32_t first, uint64_t* __restrict__ seeds,
+                     uint32_t* __restrict__ tables)
+{
+    if (threadIdx.x < p.n) seeds[first + threadIdx.x] = p.seeds[threadIdx.x];
+    if (p.with_tables)
+        for (uint32_t q = threadIdx.x; q < p.n * kTableSize; q += blockDim.x)
+            tables[(size_t)first * kTableSize + q] = p.tables[q];
+}
+
+// ---------------------------------------------------------------------------
 // K0 init: s(site) = [x0 < thr], x0 = word 0 of
 // Philox(ctr = (site,0,0,INIT), key = seed), thr = floor(rho0 * 2^32) in [0, 2^32].
 // u8: one thread writes 16 consecutive sites (one 16-byte store).

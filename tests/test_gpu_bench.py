@@ -30,8 +30,8 @@ def test_bench_line_has_the_contract_keys():
     assert "workload" in d["config"] and "model" not in d["config"]
     assert d["value"] > 0 and d["e2e"]["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] == 1024 * 1024 and d["e2e"]["d2h_bytes_per_step"] > 1024 * 1024
-    # init + density + order + 16 phases per MCS + finalize, per step, warm-up excluded
-    assert d["gpu_launches"] == 2 * (1 + 1 + 1 + 16 * 20 + 1)
+    # (seed upload + init) + (seed/table upload + density + order + 16 phases per MCS + finalize), per step
+    assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 1 + 16 * 20 + 1))
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
     a = r["alu_context"]                                  # the draws against the Philox-only ceiling
@@ -56,7 +56,7 @@ def test_bench_line_for_the_papers_schedule():
     """--order dtile: same contract line, 4 launches per MCS, no class-order kernel."""
     d = run_bench("--order", "dtile", "--no-cpu-baseline")
     assert d["config"]["order_mode"] == "dtile" and d["config"]["variant"] == 10
-    assert d["gpu_launches"] == 2 * (1 + 1 + 4 * 20 + 1)
+    assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 4 * 20 + 1))
     r = d["roofline"]
     assert r["algorithmic_bytes_per_launch"] == 1024 * 1024 * 1.25 and "dtile_part_kernel" in r["kernel"]
     assert d["value"] > 0 and d["e2e"]["value"] > 0 and 0.0 <= d["final_rho_C"] <= 1.0
