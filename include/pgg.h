@@ -148,6 +148,28 @@ int32_t pgg_run_ensemble(void* d_lats, int32_t fmt, uint32_t B, uint32_t L, cons
                          double K, const uint64_t* h_seeds, int32_t order_mode, double rho0,
                          uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts, void* stream);
 
+/* ---- The prisoner's dilemma (section VI): "the described parallelization scheme can be
+ * easily adapted so that ... other evolutionary games on the square lattice can be performed, such as
+ * ... the well-known prisoner's dilemma game ... played in a pairwise manner, not in groups.  As a
+ * consequence, the memory needed ... is one line outward less in each direction".  The paper gives no
+ * payoff matrix; readings (G1-G4):
+ *  G1 x plays one two-player game with each of its four nearest neighbours (not with itself); a pair
+ *     earns C-C: R, C-D: S, D-C: T, D-D: P; Pi_x = the sum of its four games.  (R = 1, S = P = 0, T = b
+ *     is the weak dilemma of the literature the paper cites.)
+ *  G2 the elementary step, the Fermi rule (Eq. 3), the 16-sublattice schedule and the draws are those
+ *     of pgg_sweep.
+ *  G3 with n_z = cooperators among the four neighbours of z: Pi_z = s_z ? R n_z + S (4 - n_z)
+ *     : T n_z + P (4 - n_z); thresholds T[s_x*25 + n_x*5 + n_y] for s_y = 1 - s_x, in IEEE double:
+ *     z = (Pi_x - Pi_y)/K; W = 1/(1+exp(z)); v = W * 2^32; T = v >= 4294967295 ? 0xFFFFFFFF : floor(v).
+ *  G4 a step reads within Manhattan distance 2 of x.
+ * pgg_pd_build_accept_table: pure host function, h_out50 = 50 uint32.  pgg_pd_sweep: arguments and
+ * errors as pgg_sweep with (R, S, T, P) in place of r; PGG_ORDER_IID / PGG_ORDER_PERM only; runs on the
+ * LEAN kernel where it is supported (L = 1024 .. 32768, a power of two), else on V0.                    */
+int32_t pgg_pd_build_accept_table(double R, double S, double T, double P, double K, uint32_t* h_out50);
+int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, double T, double P, double K,
+                     uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
+                     void* stream);
+
 /* The 16 phase classes of MCS t, computed by the library's own
  * device kernel and copied back; h_out16: host array of 16 bytes.  Synchronises
  * `stream`.  For tests of step a1.  PGG_ORDER_DTILE has no classes:

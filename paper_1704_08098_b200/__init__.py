@@ -38,6 +38,9 @@ SIGNATURES = {
     "pgg_run_ensemble": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_uint32, _f64p, C.c_double,
                                      _u64p, C.c_int32, C.c_double, C.c_uint32, C.c_uint32, C.c_void_p,
                                      C.c_void_p]),
+    "pgg_pd_build_accept_table": (C.c_int32, [C.c_double] * 5 + [_u32p]),
+    "pgg_pd_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32] + [C.c_double] * 5 +
+                     [C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]),
     "pgg_phase_classes": (C.c_int32, [C.c_uint64, C.c_uint32, C.c_int32, _u8p, C.c_void_p]),
     "pgg_set_variant": (C.c_int32, [C.c_int32]),
     "pgg_get_variant_used": (C.c_int32, []),
@@ -116,6 +119,19 @@ def pgg_run_ensemble(d_lats, fmt: int, B: int, L: int, h_r, K: float, h_seeds, o
     s = (C.c_uint64 * B)(*[int(x) for x in h_seeds])
     _check(lib().pgg_run_ensemble(_ptr(d_lats), fmt, B, L, r, K, s, order_mode, rho0, t_begin, n_mcs,
                                   _ptr(d_counts), _stream(stream)))
+
+
+def pgg_pd_build_accept_table(R: float, S: float, T: float, P: float, K: float):
+    """-> list of 50 thresholds of the prisoner's dilemma (host function, no CUDA)."""
+    out = (C.c_uint32 * 50)()
+    _check(lib().pgg_pd_build_accept_table(R, S, T, P, K, out))
+    return list(out)
+
+
+def pgg_pd_sweep(d_lat, fmt: int, L: int, R: float, S: float, T: float, P: float, K: float, seed: int,
+                 order_mode: int, t_begin: int, n_mcs: int, d_counts=None, stream=None) -> None:
+    _check(lib().pgg_pd_sweep(_ptr(d_lat), fmt, L, R, S, T, P, K, seed, order_mode, t_begin, n_mcs,
+                              _ptr(d_counts), _stream(stream)))
 
 
 def pgg_phase_classes(seed: int, t: int, order_mode: int, stream=None):

@@ -148,17 +148,21 @@ int32_t launch_density(const uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t 
 }
 
 // The sweep proper for B lattices (B = 1: pgg_sweep).
+// game = pgg::kGamePGG: h_r[b] = synergy factor of lattice b.  game = pgg::kGamePD (B = 1): h_r = {R, S, T, P}.
 int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const double* h_r, double K,
                    const uint64_t* h_seeds, int32_t order_mode, double rho0, uint32_t t_begin,
-                   uint32_t n_mcs, uint64_t* d_counts, cudaStream_t stream)
+                   uint32_t n_mcs, uint64_t* d_counts, cudaStream_t stream, int game = pgg::kGamePGG)
 {
+    const bool pd = game == pgg::kGamePD;
+    if (pd && order_mode == PGG_ORDER_DTILE)
+        return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs under the 16-sublattice schedule only");
     if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM && order_mode != PGG_ORDER_DTILE)
         return fail(PGG_ERR_UNSUPPORTED, "unknown order_mode %d", order_mode);
     if (order_mode == PGG_ORDER_DTILE && L % 8 != 0)
         return fail(PGG_ERR_BAD_L, "L = %u: the double tiling schedule needs L %% 8 == 0 (PAPER.md:93)", L);
     if (!(K > 0.0) || !std::isfinite(K)) return fail(PGG_ERR_BAD_PARAM, "K must be finite and > 0");
-    for (uint32_t b = 0; b < B; ++b)
-        if (!std::isfinite(h_r[b])) return fail(PGG_ERR_BAD_PARAM, "r[%u] is not finite", b);
+    for (uint32_t b = 0; b < (pd ? 4u : B); ++b)
+        if (!std::isfinite(h_r[b])) return fail(PGG_ERR_BAD_PARAM, pd ? "payoff %u (R, S, T, P) is not finite" : "r[%u] is not finite", b);
     if ((unsigned long long)t_begin + n_mcs > 4294967296ull)
         return fail(PGG_ERR_BAD_PARAM, "t_begin + n_mcs exceeds 2^32");
 
@@ -189,6 +193,14 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
                 : !stream_pays ? PGG_VARIANT_V0
                 : (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
     }
+    if (pd) {  // two kernels carry the second game: LEAN where it runs, else the general V0
+        const int asked = g_variant.load();
+        if (asked != PGG_VARIANT_AUTO && asked != PGG_VARIANT_V0 && asked != PGG_VARIANT_LEAN)
+            return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs on variants V0 and LEAN only (asked: %d)", asked);
+        variant = (asked != PGG_VARIANT_V0 && pgg::lean_supported(fmt, L)) ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;
+        if (asked == PGG_VARIANT_LEAN && variant != PGG_VARIANT_LEAN)
+            return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", asked, fmt, L);
+    }
     if (variant == PGG_VARIANT_RESIDENT && !res_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_LEAN && !pgg::lean_supported(fmt, L))
@@ -205,7 +217,8 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     // per-lattice seeds and acceptance tables
     std::vector<uint32_t> h_tables((size_t)B * pgg::kTableSize);
     for (uint32_t b = 0; b < B; ++b) {
-        int32_t rc = pgg_build_accept_table(h_r[b], K, h_tables.data() + (size_t)b * pgg::kTableSize);
+        int32_t rc = pd ? pgg_pd_build_accept_table(h_r[0], h_r[1], h_r[2], h_r[3], K, h_tables.data() + (size_t)b * pgg::kTableSize)
+                        : pgg_build_accept_table(h_r[b], K, h_tables.data() + (size_t)b * pgg::kTableSize);
         if (rc != PGG_OK) return rc;
     }
     uint64_t* d_seeds = nullptr;
@@ -321,7 +334,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
                 if (variant == PGG_VARIANT_LEAN) {
-                    pgg::lean_launch(lplan, fmt, a, m, k, B, stream);
+                    pgg::lean_launch(lplan, fmt, a, m, k, B, stream, game);
                 } else if (variant == PGG_VARIANT_DYN) {
                     pgg::dyn_launch(rplan, a, m, k, B, stream);
                 } else if (variant == PGG_VARIANT_SPLIT) {
@@ -337,7 +350,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
                 } else {
                     const uint32_t n_cls = (L / 4) * (L / 4);
                     dim3 grid((n_cls + 255) / 256, B);
-                    if (fmt == PGG_FMT_U8)
+                    if (pd && fmt == PGG_FMT_U8)
+                        pgg::phase_v0_kernel<pgg::kFmtU8, pgg::kGamePD><<<grid, 256, 0, stream>>>(a, m, k);
+                    else if (pd)
+                        pgg::phase_v0_kernel<pgg::kFmtBits, pgg::kGamePD><<<grid, 256, 0, stream>>>(a, m, k);
+                    else if (fmt == PGG_FMT_U8)
                         pgg::phase_v0_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, m, k);
                     else
                         pgg::phase_v0_kernel<pgg::kFmtBits><<<grid, 256, 0, stream>>>(a, m, k);
@@ -376,6 +393,37 @@ int32_t pgg_build_accept_table(double r, double K, uint32_t* h_out153)
         }
     }
     return PGG_OK;
+}
+
+int32_t pgg_pd_build_accept_table(double R, double S, double T, double P, double K, uint32_t* h_out50)
+{
+    if (h_out50 == nullptr) return fail(PGG_ERR_NULL, "out50 is NULL");
+    if (!std::isfinite(R) || !std::isfinite(S) || !std::isfinite(T) || !std::isfinite(P) || !std::isfinite(K) || !(K > 0.0))
+        return fail(PGG_ERR_BAD_PARAM, "R, S, T, P and K must be finite, K > 0");
+    // Eq. (3), for the pair-game payoffs of PAPER.md:131 (readings G1, G3 in pgg.h)
+    for (int sx = 0; sx <= 1; ++sx)
+        for (int nx = 0; nx <= 4; ++nx)
+            for (int ny = 0; ny <= 4; ++ny) {
+                auto pay = [&](int s, int n) { return s == 1 ? R * (double)n + S * (double)(4 - n) : T * (double)n + P * (double)(4 - n); };
+                volatile double px = pay(sx, nx);
+                volatile double py = pay(1 - sx, ny);
+                volatile double z = (px - py) / K;
+                volatile double W = 1.0 / (1.0 + std::exp(z));
+                const double v = W * 4294967296.0;
+                h_out50[sx * 25 + nx * 5 + ny] = (v >= 4294967295.0) ? 0xFFFFFFFFu : (uint32_t)std::floor(v);
+            }
+    return PGG_OK;
+}
+
+int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, double T, double P, double K,
+                     uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
+                     void* stream)
+{
+    int32_t rc = check_lattice_args(d_lat, fmt, L);
+    if (rc != PGG_OK) return rc;
+    const double h_pd[4] = {R, S, T, P};
+    return run_sweeps(static_cast<uint8_t*>(d_lat), fmt, 1, L, h_pd, K, &seed, order_mode, -1.0, t_begin, n_mcs,
+                      d_counts, static_cast<cudaStream_t>(stream), pgg::kGamePD);
 }
 
 int32_t pgg_init_lattice(void* d_lat, int32_t fmt, uint32_t L, double rho0, uint64_t seed, void* stream)

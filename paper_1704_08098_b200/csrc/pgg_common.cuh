@@ -11,6 +11,12 @@ namespace pgg {
 constexpr int kFmtU8 = 0;
 constexpr int kFmtBits = 1;
 constexpr int kTableSize = 153;  // 3 values of ds x 51 values of dA
+// The game whose payoffs decide the step.  kGamePD is the prisoner's dilemma the paper names as the
+// first other game its scheme adapts to (readings G1-G4 in include/pgg.h): its 50
+// thresholds, indexed s_x*25 + n_x*5 + n_y, sit at the front of the lattice's 153-entry table slot.
+constexpr int kGamePGG = 0;
+constexpr int kGamePD = 1;
+constexpr int kPdTableSize = 50;
 
 // One phase launch covers B lattices (B = 1 for pgg_sweep).  Per-lattice data
 // live in device arrays indexed by the lattice number b.
@@ -87,6 +93,13 @@ __device__ __forceinline__ int payoff_A(const Lat& lat, int i, int j)
                    lat.get(i + 1, j + 1);
     const int ax = lat.get(i - 2, j) + lat.get(i + 2, j) + lat.get(i, j - 2) + lat.get(i, j + 2);
     return 5 * c + 2 * (nn + dg) + ax;
+}
+
+// Prisoner's dilemma: number of cooperators among the four nearest neighbours of (i,j) (G3).
+template <class Lat>
+__device__ __forceinline__ int pd_neighbour_count(const Lat& lat, int i, int j)
+{
+    return lat.get(i - 1, j) + lat.get(i + 1, j) + lat.get(i, j - 1) + lat.get(i, j + 1);
 }
 
 __device__ __forceinline__ int table_index(int dA, int ds)

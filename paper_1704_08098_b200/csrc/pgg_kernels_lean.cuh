@@ -118,7 +118,8 @@ __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar)
 
 // SRC = layout of the lattice in global memory (kFmtU8 / kFmtBits); the ring is always bits.
 // Warps 0..15: workers.  Warp 16: producer (bulk copies).  Warps 17..20 (uint8 only): packers.
-template <int SRC>
+// GAME = kGamePGG (the 14-read payoff stencil) or kGamePD (neighbour counts of x and y).
+template <int SRC, int GAME = kGamePGG>
 __global__ void __launch_bounds__(SRC == kFmtU8 ? kLeanThreadsU8 : kLeanThreads, 1)
 phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
 {
@@ -302,10 +303,24 @@ phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
             const int soff = (int)(w.x & 0x1FFFFFFFu), sx = (int)((w.x >> 29) & 1u);
             const uint32_t dir = w.x >> 30;
             const int col = soff & colmask;
-            const int dA = (col < 3 || col > colmask - 3)
-                               ? ring_stencil_fr<kFmtBits>(soff, dir, sx, ring0, 0, colmask)
-                               : ring_stencil<kFmtBits, false>(soff, dir, sx, ring0, eoff, 0);
-            if (w.z < tbl[sx * 102 + dA + 25]) {  // table_index(dA, ds) with ds = 2 s_x - 1
+            int idx_t;
+            if (GAME == kGamePD) {
+                // n_x, n_y: the four neighbours of x and of y = x + e; columns wrap inside the row
+                const int ps = colmask + 1, rowb = soff - col;
+                auto N4 = [&](int rb, int c) {
+                    return ring_get<kFmtBits>(ring0, rb - ps + c) + ring_get<kFmtBits>(ring0, rb + ps + c) +
+                           ring_get<kFmtBits>(ring0, rb + ((c - 1) & colmask)) + ring_get<kFmtBits>(ring0, rb + ((c + 1) & colmask));
+                };
+                const int yr = rowb + (dir == 0u ? -ps : dir == 1u ? ps : 0);
+                const int yc = (col + (dir == 2u ? -1 : dir == 3u ? 1 : 0)) & colmask;
+                idx_t = sx * 25 + N4(rowb, col) * 5 + N4(yr, yc);
+            } else {
+                const int dA = (col < 3 || col > colmask - 3)
+                                   ? ring_stencil_fr<kFmtBits>(soff, dir, sx, ring0, 0, colmask)
+                                   : ring_stencil<kFmtBits, false>(soff, dir, sx, ring0, eoff, 0);
+                idx_t = sx * 102 + dA + 25;  // table_index(dA, ds) with ds = 2 s_x - 1
+            }
+            if (w.z < tbl[idx_t]) {
                 if (SRC == kFmtU8)
                     lat[w.y] = (uint8_t)(1 - sx);
                 else
@@ -472,6 +487,10 @@ inline int lean_plan(int fmt, uint32_t L, uint32_t B, LeanPlan* p)
     if (e != cudaSuccess) return (int)e;
     e = cudaFuncSetAttribute((const void*)phase_lean_kernel<kFmtBits>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
     if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute((const void*)phase_lean_kernel<kFmtU8, kGamePD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute((const void*)phase_lean_kernel<kFmtBits, kGamePD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+    if (e != cudaSuccess) return (int)e;
     uint32_t lg = 0;
     while ((1u << lg) < L) ++lg;
     p->lg2L = lg;
@@ -480,15 +499,18 @@ inline int lean_plan(int fmt, uint32_t L, uint32_t B, LeanPlan* p)
     const uint32_t wpr = L / 32;
     p->R = wpr >= 512 ? 1u : 512u / wpr;
     p->n_seg = wpr > 512 ? wpr / 512 : 1u;
-    if (const char* s = getenv("PGG_LEAN_WORDS")) {  // words per lane and step: 1 (default) or 2
-        if (atoi(s) == 2 && (L / 4) % (2 * p->R) == 0) { p->R *= 2; p->n_seg *= 2; }
-    }
+    uint32_t per_lat = (uint32_t)sms / B;
+    if (per_lat < 1) per_lat = 1;
+    // Two words per lane and step (R doubles) halve the per-step overhead: 46.5 against 50.4 us per phase on
+    // bit-packed C5.  Only where a band keeps >= 8 steps (the ring fills once per band) and, for uint8, never:
+    // there the doubled ring chunks squeeze the staging slots (77 against 64 us).
+    uint32_t words = (fmt == kFmtBits && (L / 4) % (2 * p->R) == 0 && (L / 4) / (2 * p->R) >= 8 * per_lat) ? 2u : 1u;
+    if (const char* s = getenv("PGG_LEAN_WORDS")) words = (atoi(s) == 2 && (L / 4) % (2 * p->R) == 0) ? 2u : 1u;
+    if (words == 2) { p->R *= 2; p->n_seg *= 2; }
     p->RC = 4 * p->R;
     p->n_steps_total = (L / 4) / p->R;
     // (Two CTAs per SM fit the bit-packed ring, but need <= 60 registers per thread: the spills cost
     // more than the second CTA hides -- 46 against 40 us per phase, profiles/r2_lean_notes.md.)
-    uint32_t per_lat = (uint32_t)sms / B;
-    if (per_lat < 1) per_lat = 1;
     p->nb = p->n_steps_total < per_lat ? p->n_steps_total : per_lat;
     const uint32_t avail = (uint32_t)smem_optin - 256 - kLeanFixedBytes;
     const uint32_t chunk_bits_bytes = p->RC * p->pitch;
@@ -539,7 +561,7 @@ inline int lean_plan(int fmt, uint32_t L, uint32_t B, LeanPlan* p)
 }
 
 inline void lean_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t m, uint32_t k, uint32_t B,
-                        cudaStream_t stream)
+                        cudaStream_t stream, int game = kGamePGG)
 {
     static const bool pdl = [] { const char* e = getenv("PGG_PDL"); return e == nullptr || atoi(e) != 0; }();
     cudaLaunchConfig_t cfg{};
@@ -552,7 +574,12 @@ inline void lean_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (fmt == kFmtU8)
+    if (game == kGamePD) {
+        if (fmt == kFmtU8)
+            cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtU8, kGamePD>, a, m, k, p);
+        else
+            cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtBits, kGamePD>, a, m, k, p);
+    } else if (fmt == kFmtU8)
         cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtU8>, a, m, k, p);
     else
         cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtBits>, a, m, k, p);

@@ -195,7 +195,7 @@ finalize_counts_kernel(unsigned long long* __restrict__ counts, uint32_t n_mcs,
 // Race-free in place (S1): the step reads only sites within Manhattan distance
 // 3 of x, other active sites are >= 4 away, and it writes only x.
 // ---------------------------------------------------------------------------
-template <int FMT>
+template <int FMT, int GAME = kGamePGG>
 __global__ void __launch_bounds__(256)
 phase_v0_kernel(PhaseArgs a, uint32_t m, uint32_t k)
 {
@@ -224,8 +224,12 @@ phase_v0_kernel(PhaseArgs a, uint32_t m, uint32_t k)
             if (sy != sx) {
                 const int yi = i + (dir == 0 ? -1 : dir == 1 ? 1 : 0);
                 const int yj = j + (dir == 2 ? -1 : dir == 3 ? 1 : 0);
-                const int dA = payoff_A(lat, i, j) - payoff_A(lat, yi, yj);
-                if (u < table[table_index(dA, sx - sy)]) {
+                // public goods game: the difference of the integer payoffs A; prisoner's dilemma
+                // (PAPER.md:131): the cooperating neighbours of x and of y, radius 2 only
+                const int idx_t = GAME == kGamePD
+                                      ? sx * 25 + (s_up + s_dn + s_lf + s_rt) * 5 + pd_neighbour_count(lat, yi, yj)
+                                      : table_index(payoff_A(lat, i, j) - payoff_A(lat, yi, yj), sx - sy);
+                if (u < table[idx_t]) {
                     lat.flip_to(i, j, sy);
                     delta = sy - sx;
                 }

@@ -72,6 +72,7 @@ def decay(r, seeds, L=2048, n_mcs=100000, K=0.5, rho0=0.5, order=ORDER_IID, fmt=
     """-> list of rows {t, rho, rho_err, delta_eff, delta_err}: seed average of rho_C(t), error from the
     scatter between seeds; delta_eff(t) between t/8 and t with a seed-jackknife error."""
     tr = run_traces(L, [r] * len(seeds), seeds, K, rho0, n_mcs, order, fmt).astype(np.float64) / (L * L)
+    decay.last_fit = decay_fit(tr, n_mcs)      # read by main(): the last-decade fit of the same traces
     rows = []
     n = len(seeds)
     for t in log_times(n_mcs):
@@ -91,6 +92,28 @@ def decay(r, seeds, L=2048, n_mcs=100000, K=0.5, rho0=0.5, order=ORDER_IID, fmt=
             row.update(delta_eff=full, delta_err=err)
         rows.append(row)
     return rows
+
+
+def decay_fit(tr, n_mcs, t_lo=None):
+    """Least-squares slope of ln rho(t) against ln t over the log-spaced times in [t_lo, n_mcs] (default: the
+    last decade), rho = seed mean; error from a jackknife over the seeds.  tr: [n_seeds, n_mcs] densities."""
+    t_lo = t_lo or max(1, n_mcs // 10)
+    ts = np.array([t for t in log_times(n_mcs) if t >= t_lo])
+    x = np.log(ts.astype(np.float64))
+
+    def slope(sel):
+        y = tr[sel][:, ts - 1].mean(axis=0)
+        if (y <= 0).any():
+            return float("nan")
+        return -float(np.polyfit(x, np.log(y), 1)[0])
+    n = tr.shape[0]
+    full = slope(slice(None))
+    if n > 1:
+        jk = np.array([slope([i for i in range(n) if i != j]) for j in range(n)])
+        err = float(math.sqrt((n - 1) / n * ((jk - jk.mean()) ** 2).sum()))
+    else:
+        err = 0.0
+    return {"t_lo": int(ts[0]), "t_hi": int(ts[-1]), "points": int(len(ts)), "delta": full, "delta_err": err}
 
 
 def fig5(order=ORDER_DTILE, n_mcs=2000, Ls=(32, 64, 128, 256, 512, 1024, 2048, 4096), r=3.98, K=0.5, seed=1):
@@ -139,7 +162,7 @@ def main():
         rows = decay(args.r, seeds, args.L or 2048, args.mcs or 100000, order=order,
                      fmt=FMT_BITS if args.fmt == "bits" else FMT_U8)
         print(json.dumps({"what": "decay", "order": args.order, "r": args.r, "L": args.L or 2048, "fmt": args.fmt,
-                          "mcs": args.mcs or 100000, "seeds": seeds, "rows": rows}))
+                          "mcs": args.mcs or 100000, "seeds": seeds, "last_decade_fit": decay.last_fit, "rows": rows}))
 
 
 if __name__ == "__main__":

@@ -125,3 +125,24 @@ def test_variant_support_table():
     assert sup(pgg.VARIANT_SPLIT, pgg.FMT_U8, 2048) and not sup(pgg.VARIANT_SPLIT, pgg.FMT_BITS, 2048)
     assert sup(pgg.VARIANT_DYN, pgg.FMT_U8, 2048) and not sup(pgg.VARIANT_DYN, pgg.FMT_BITS, 2048)
     assert not sup(99, pgg.FMT_U8, 64)
+
+
+def test_prisoners_dilemma_tables_equal_oracle_tables_and_validation():
+    """The library's 50 thresholds of the prisoner's dilemma (G3) against the oracle's,
+    built independently; argument validation of the two entry points (no GPU needed: all fail first)."""
+    import oracle as orc
+    for (R, S, T, P, K) in ((1.0, 0.0, 1.3, 0.0, 0.1), (3.0, -0.5, 4.25, 0.75, 0.5), (1.0, 0.0, 2.0, 0.0, 1e-3),
+                            (1.0, 0.0, 1.0, 0.0, 50.0)):
+        assert pgg.pgg_pd_build_accept_table(R, S, T, P, K) == orc.pd_accept_table(R, S, T, P, K).tolist()
+    h = pgg.lib()
+    out = (C.c_uint32 * 50)()
+    assert h.pgg_pd_build_accept_table(1.0, 0.0, 1.3, 0.0, 0.0, out) == pgg.ERR_BAD_PARAM
+    assert h.pgg_pd_build_accept_table(float("nan"), 0.0, 1.3, 0.0, 0.1, out) == pgg.ERR_BAD_PARAM
+    assert h.pgg_pd_build_accept_table(1.0, 0.0, 1.3, 0.0, 0.1, None) == pgg.ERR_NULL
+    fake = 0x1000
+    args = (1.0, 0.0, 1.3, 0.0, 0.1, 1)
+    assert h.pgg_pd_sweep(None, 0, 64, *args, 0, 0, 1, None, None) == pgg.ERR_NULL
+    assert h.pgg_pd_sweep(fake, 0, 6, *args, 0, 0, 1, None, None) == pgg.ERR_BAD_L
+    assert h.pgg_pd_sweep(fake, 0, 64, 1.0, 0.0, float("inf"), 0.0, 0.1, 1, 0, 0, 1, None, None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_pd_sweep(fake, 0, 64, 1.0, 0.0, 1.3, 0.0, -1.0, 1, 0, 0, 1, None, None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_pd_sweep(fake, 0, 64, *args, pgg.ORDER_DTILE, 0, 1, None, None) == pgg.ERR_UNSUPPORTED
