@@ -96,8 +96,10 @@ enum {
                                 every phase of the call in one launch                  */
     PGG_VARIANT_DTILE = 10,  /* reported by pgg_get_variant_used() after a PGG_ORDER_DTILE
                                 sweep (one thread per 4x4 domain); not selectable       */
-    PGG_VARIANT_LEAN = 11    /* L = 1024 .. 32768, a power of two: whole rows streamed, packed to
+    PGG_VARIANT_LEAN = 11,   /* L = 1024 .. 32768, a power of two: whole rows streamed, packed to
                                 bits on arrival (uint8), scan / draw / stencil on a bit ring   */
+    PGG_VARIANT_PERSIST = 12 /* LEAN, bit-packed, <= 148 lattices: every phase of up to 4096 MCS in ONE
+                                cooperative launch, a per-lattice barrier between phases           */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:

@@ -195,9 +195,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     }
     if (pd) {  // two kernels carry the second game: LEAN where it runs, else the general V0
         const int asked = g_variant.load();
-        if (asked != PGG_VARIANT_AUTO && asked != PGG_VARIANT_V0 && asked != PGG_VARIANT_LEAN)
-            return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs on variants V0 and LEAN only (asked: %d)", asked);
-        variant = (asked != PGG_VARIANT_V0 && pgg::lean_supported(fmt, L)) ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;
+        if (asked != PGG_VARIANT_AUTO && asked != PGG_VARIANT_V0 && asked != PGG_VARIANT_LEAN && asked != PGG_VARIANT_PERSIST)
+            return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs on variants V0, LEAN and PERSIST only (asked: %d)", asked);
+        variant = asked == PGG_VARIANT_PERSIST ? PGG_VARIANT_PERSIST
+                : (asked != PGG_VARIANT_V0 && pgg::lean_supported(fmt, L)) ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;
         if (asked == PGG_VARIANT_LEAN && variant != PGG_VARIANT_LEAN)
             return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", asked, fmt, L);
     }
@@ -205,6 +206,8 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_LEAN && !pgg::lean_supported(fmt, L))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
+    if (variant == PGG_VARIANT_PERSIST && !pgg::lean_persist_supported(fmt, L, B))
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u, B %u", variant, fmt, L, B);
     const bool split_ok = pgg::split_supported(fmt, L);
     if ((variant == PGG_VARIANT_BAND && !band_ok) || (variant == PGG_VARIANT_RING && !ring_ok) ||
         (variant == PGG_VARIANT_SPLIT && !split_ok) || (variant == PGG_VARIANT_DYN && !pgg::dyn_supported(fmt, L)))
@@ -312,7 +315,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     }
 
     pgg::LeanPlan lplan;
-    if (variant == PGG_VARIANT_LEAN) {
+    unsigned int* d_gbar = nullptr;
+    if (variant == PGG_VARIANT_PERSIST) {
+        PGG_CUDA(tmp.alloc((void**)&d_gbar, sizeof(unsigned int) * B));
+    }
+    if (variant == PGG_VARIANT_LEAN || variant == PGG_VARIANT_PERSIST) {
         int32_t rc = pgg::lean_plan(fmt, L, B, &lplan);
         if (rc != 0) return fail(PGG_ERR_CUDA, "lean kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
     }
@@ -328,6 +335,12 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         PGG_LAUNCHED();
         if (variant == PGG_VARIANT_RESIDENT) {  // all 16 * n_chunk phases in one launch
             pgg::resident_launch(resplan, fmt, a, m0, n_chunk, B, stream);
+            PGG_LAUNCHED();
+            continue;
+        }
+        if (variant == PGG_VARIANT_PERSIST) {   // likewise, cooperative: a barrier per phase instead of a launch
+            PGG_CUDA(cudaMemsetAsync(d_gbar, 0, sizeof(unsigned int) * B, stream));
+            PGG_CUDA(pgg::lean_persist_launch(lplan, a, m0, n_chunk, B, d_gbar, stream, game));
             PGG_LAUNCHED();
             continue;
         }
@@ -497,7 +510,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_LEAN || variant == PGG_VARIANT_DTILE || variant == 3)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_PERSIST || variant == PGG_VARIANT_DTILE || variant == 3)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -517,6 +530,7 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_DYN) return pgg::dyn_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_RESIDENT) return pgg::resident_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_LEAN) return pgg::lean_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_PERSIST) return pgg::lean_persist_supported(fmt, L, 1) ? 1 : 0;
     return 0;
 }
 

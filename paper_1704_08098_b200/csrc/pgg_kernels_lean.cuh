@@ -119,9 +119,11 @@ __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar)
 // SRC = layout of the lattice in global memory (kFmtU8 / kFmtBits); the ring is always bits.
 // Warps 0..15: workers.  Warp 16: producer (bulk copies).  Warps 17..20 (uint8 only): packers.
 // GAME = kGamePGG (the 14-read payoff stencil) or kGamePD (neighbour counts of x and y).
-template <int SRC, int GAME = kGamePGG>
-__global__ void __launch_bounds__(SRC == kFmtU8 ? kLeanThreadsU8 : kLeanThreads, 1)
-phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
+// PERSIST: called once per phase from the persistent kernel (no programmatic-dependent-launch fences;
+// the mbarriers are initialised afresh, which is legal because every warp has passed the closing
+// __syncthreads of the previous phase).
+template <int SRC, int GAME, bool PERSIST>
+__device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint32_t k, const LeanPlan& g)
 {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int pitch = (int)g.pitch, RC = (int)g.RC;
@@ -144,7 +146,7 @@ phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
     const uint32_t bar_full = smem_u32(bars), bar_empty = bar_full + 8u * kLeanMaxSlots;   // of the bit ring's chunks
     const uint32_t bar_sfull = bar_empty + 8u * kLeanMaxSlots, bar_sempty = bar_sfull + 8u * kLeanMaxSlots;  // of the staging slots
 
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (!PERSIST) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (int q = threadIdx.x; q < kTableSize; q += blockDim.x)
         tbl[q] = a.tables[(size_t)b * kTableSize + q];
     if (threadIdx.x == 0) {
@@ -164,7 +166,7 @@ phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
         eoff[4] = 1;   eoff[5] = 1;  eoff[6] = ps; eoff[7] = ps;
     }
     __syncthreads();
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (!PERSIST) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
     const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
 
@@ -179,6 +181,9 @@ phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
 
     if (warp == kLeanConsumers) {
         // ---------------- producer warp ----------------
+        // PERSIST: the flips of the previous phase were made by other SMs through the generic proxy; the
+        // grid barrier has ordered them before this point, this fence orders them before the bulk copies
+        if (PERSIST) asm volatile("fence.proxy.async.global;" ::: "memory");
         int grow = row_c0 < 0 ? row_c0 + (int)L : row_c0;  // lattice row of the current chunk's first row
         if (SRC == kFmtU8) {
             const uint32_t stage_s = smem_u32(smem_raw + stage_off);
@@ -465,6 +470,48 @@ phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
         atomicAdd(a.deltas + (size_t)b * a.n_mcs + m, (unsigned long long)(long long)delta_cta);
 }
 
+template <int SRC, int GAME = kGamePGG>
+__global__ void __launch_bounds__(SRC == kFmtU8 ? kLeanThreadsU8 : kLeanThreads, 1)
+phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
+{
+    lean_phase<SRC, GAME, false>(a, m, k, g);
+}
+
+// ---------------------------------------------------------------------------
+// PERSIST: every phase of n_mcs MCS (16 n_mcs phases) in ONE cooperative launch, bit-packed source.
+// ("minimizing the need to access global memory" -- and, on this machine, the launches.)
+// The lattice stays where it is (L2-resident for the sizes this is used for); between two phases the
+// CTAs of one lattice meet at a barrier in global memory -- lattices of an ensemble never wait for
+// each other.  A phase reads what the previous one wrote within radius 3 of every site, so the
+// barrier is the method's own dependency, not an artefact; what it saves is the launch, the drain of
+// the grid and the refill of 148 empty pipelines behind a grid-wide dependency.
+// gbar[b] counts arrivals of lattice b's CTAs (zeroed by the host); after phase p it reaches (p+1) nb.
+// ---------------------------------------------------------------------------
+template <int GAME>
+__global__ void __launch_bounds__(kLeanThreads, 1)
+sweep_lean_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, LeanPlan g, unsigned int* __restrict__ gbar)
+{
+    const uint32_t n_phases = 16u * n_mcs;
+    unsigned int* bar = gbar + blockIdx.y;
+    for (uint32_t p = 0; p < n_phases; ++p) {
+        lean_phase<kFmtBits, GAME, true>(a, m0 + (p >> 4), p & 15u, g);  // ends with __syncthreads()
+        if (p + 1 == n_phases) break;
+        if (threadIdx.x == 0) {
+            __threadfence();  // this CTA's flips (atomics) and counts before its arrival
+            atomicAdd(bar, 1u);
+            const unsigned int target = (p + 1u) * g.nb;
+            unsigned int seen, spins = 0;
+            for (;;) {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+                if (seen >= target) break;
+                __nanosleep(40);
+                if (++spins > (1u << 24)) __trap();  // ~1 s: a lost CTA must not hang the device
+            }
+        }
+        __syncthreads();
+    }
+}
+
 // ---------------------------------------------------------------------------
 // Host side
 // ---------------------------------------------------------------------------
@@ -490,6 +537,10 @@ inline int lean_plan(int fmt, uint32_t L, uint32_t B, LeanPlan* p)
     e = cudaFuncSetAttribute((const void*)phase_lean_kernel<kFmtU8, kGamePD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
     if (e != cudaSuccess) return (int)e;
     e = cudaFuncSetAttribute((const void*)phase_lean_kernel<kFmtBits, kGamePD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute((const void*)sweep_lean_kernel<kGamePGG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute((const void*)sweep_lean_kernel<kGamePD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 256);
     if (e != cudaSuccess) return (int)e;
     uint32_t lg = 0;
     while ((1u << lg) < L) ++lg;
@@ -583,6 +634,23 @@ inline void lean_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t
         cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtU8>, a, m, k, p);
     else
         cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtBits>, a, m, k, p);
+}
+
+// One cooperative launch for MCS [m0, m0 + n_mcs) of B lattices; d_gbar: B zeroed counters.
+inline cudaError_t lean_persist_launch(const LeanPlan& p, const PhaseArgs& a, uint32_t m0, uint32_t n_mcs, uint32_t B,
+                                       unsigned int* d_gbar, cudaStream_t stream, int game = kGamePGG)
+{
+    PhaseArgs a_ = a;
+    LeanPlan p_ = p;
+    void* args[] = {&a_, &m0, &n_mcs, &p_, &d_gbar};
+    const void* fn = game == kGamePD ? (const void*)sweep_lean_kernel<kGamePD> : (const void*)sweep_lean_kernel<kGamePGG>;
+    return cudaLaunchCooperativeKernel(fn, dim3(p.nb, B), dim3(kLeanThreads), args, p.smem_bytes, stream);
+}
+
+// Can the persistent kernel run this workload?  Bit-packed, and every CTA resident at once.
+inline bool lean_persist_supported(int fmt, uint32_t L, uint32_t B)
+{
+    return fmt == kFmtBits && lean_supported(fmt, L) && B <= 148;
 }
 
 }  // namespace pgg

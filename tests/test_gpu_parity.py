@@ -409,6 +409,7 @@ LONG_CASES = [
     ("BAND", pgg.FMT_BITS, 512, {}),                             # BAND, bit-packed (C5 packed)
     ("LEAN", pgg.FMT_U8, 1024, {}),                              # LEAN, uint8 packed to bits on chip
     ("LEAN", pgg.FMT_BITS, 1024, {}),                            # LEAN, bit-packed source
+    ("PERSIST", pgg.FMT_BITS, 1024, {}),                         # LEAN, one cooperative launch per 4096 MCS
 ]
 
 
@@ -437,7 +438,7 @@ def test_one_call_longer_than_an_order_chunk(name, fmt, L, env, monkeypatch):
 
 
 @pytest.mark.parametrize("name,fmt,L,env", LONG_CASES,
-                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits"])
+                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits", "PERSIST-bits"])
 @pytest.mark.parametrize("t0", [99900, 2**32 - 40])
 def test_streaming_kernels_late_windows(name, fmt, L, env, t0, monkeypatch):
     """SURVEY 8(d) late windows (t = 99 900) and the counter width (t_begin + m up to 2^32 - 1)
@@ -538,3 +539,40 @@ def test_lean_config5_full_size(fmt):
     ref_counts, _ = orc.sweep(ref, r, K, seed, pgg.ORDER_IID, 0, 2, n_threads=orc.max_threads())
     assert_same(to_host(d, fmt, L), ref, "C5 lattice after 2 MCS")
     assert_same(cnt.cpu().numpy().astype(np.uint64), ref_counts)
+
+
+# ---------------------------------------------------------------- PERSIST (LEAN in one cooperative launch)
+@pytest.mark.parametrize("L,n_mcs", [(1024, 6), (2048, 4), (4096, 3), (16384, 2)])
+def test_persist_parity_sizes(L, n_mcs):
+    """Every phase of the call in one launch, a barrier in global memory between phases: the same
+    lattices and counts as the oracle, from one CTA per lattice row group (L = 1024) to C5's size."""
+    fmt = pgg.FMT_BITS
+    use_variant(pgg.VARIANT_PERSIST, fmt, L)
+    for seed, r, order, rho0 in ((L + 1, 3.8, pgg.ORDER_IID, 0.5), (2**35 + L, 4.6, pgg.ORDER_PERM, 0.1)):
+        lat0 = orc.init(L, rho0, seed)
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, r, K, seed, order, 3, n_mcs, n_threads=orc.max_threads())
+        before = pgg.pgg_launch_count()
+        got, counts = gpu_sweep(lat0, fmt, r, seed, order, 3, n_mcs)
+        assert pgg.pgg_get_variant_used() == pgg.VARIANT_PERSIST
+        assert pgg.pgg_launch_count() - before == 5       # upload, density, order, ONE sweep launch, finalize
+        assert_same(got, ref, f"lattice L={L}")
+        assert_same(counts, ref_counts, f"counts L={L}")
+
+
+def test_persist_ensemble_equals_oracle():
+    """16 lattices of L = 2048 (config 3's shape): each lattice's CTAs meet at their own barrier."""
+    fmt, B, L, n_mcs = pgg.FMT_BITS, 16, 2048, 3
+    use_variant(pgg.VARIANT_PERSIST, fmt, L)
+    rs = [3.74 + 0.002 * b for b in range(B)]
+    seeds = [2**33 + 7 * b for b in range(B)]
+    d = empty_lattice(fmt, L, B)
+    cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, n_mcs, cnt)
+    torch.cuda.synchronize()
+    got = to_host(d, fmt, L)
+    for b in (0, 7, 15):
+        ref = orc.init(L, 0.5, seeds[b])
+        ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs, n_threads=orc.max_threads())
+        assert_same(got[b], ref, f"member {b}")
+        assert_same(cnt[b].cpu().numpy().astype(np.uint64), ref_counts)
