@@ -78,7 +78,7 @@ enum { PGG_FMT_U8 = 0, PGG_FMT_BITS = 1 };
 enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
 
 /* Kernel variants of the phase step (all bit-identical).
- * PGG_VARIANT_AUTO picks by measurement (profiles/r2_auto_small_lattices.md, profiles/r2_lean_notes.md):
+ * PGG_VARIANT_AUTO picks by measurement (DESIGN.md appendix B, DESIGN.md appendix B):
  * RESIDENT for L <= 320, and for L <= 512 from 3 lattices (6 at L = 512; uint8 L = 512: from 20, RING
  * below that); LEAN for the bit-packed layout at L = 1024 .. 32768 (powers of two); RING (uint8) / BAND
  * (bit-packed) for the other L >= 2048 and for uint8 L = 512, 1024; else V0.                          */

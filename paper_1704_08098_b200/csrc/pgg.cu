@@ -170,11 +170,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     const bool tile_ok = pgg::tile_supported(fmt, L);
     const bool band_ok = pgg::band_supported(fmt, L);
     const bool ring_ok = pgg::ring_supported(fmt, L);
-    // measured (profiles/r1_ring_design_notes.md): small lattices stay resident in shared memory;
+    // measured (DESIGN.md appendix A): small lattices stay resident in shared memory;
     // of the streaming kernels uint8 is fastest on RING, bit-packed on BAND
     const bool res_ok = pgg::resident_supported(fmt, L);
     if (variant == PGG_VARIANT_AUTO) {
-        // Measured rule (profiles/r2_auto_small_lattices.md, us per phase at r = 3.8).  RESIDENT takes one SM
+        // Measured rule (DESIGN.md appendix B, us per phase at r = 3.8).  RESIDENT takes one SM
         // per lattice whatever B is and grows with L^2 (1.5 us at L = 128, 2.8 at 320, 4.7 at 400, 6.9 at
         // 512); a V0 launch costs 4.2 us until B L^2 makes it throughput-bound.  So RESIDENT for L <= 320,
         // and above that from the batch size at which V0 has become slower: 3 lattices (L <= 448), 6 (L = 512).

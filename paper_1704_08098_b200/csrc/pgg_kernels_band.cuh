@@ -1,6 +1,6 @@
 // pgg_kernels_band.cuh -- the BAND phase kernel (K1 uint8, K2 bit-packed).
 //
-// Measured on B200 (profiles/r1_bulk_copy_microbench.md): cp.async.bulk copies
+// Measured on B200 (DESIGN.md appendix A): cp.async.bulk copies
 // of ~0.5 KB issued by one warp deliver only ~2.2 TB/s chip-wide, copies of
 // >= 1 KB reach 5.6-5.8 TB/s.  So the lattice is not cut into square tiles
 // (short rows, 16 % halo re-reads) but into column STRIPS of up to 8 KB, and

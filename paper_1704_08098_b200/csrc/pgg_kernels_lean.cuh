@@ -391,20 +391,21 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
         // ---- survivors of one 32-site word per lane -> Q1, lane-serially after a warp prefix sum.
         // At most 128 new entries per round (Q1 holds 160): a crowded word goes in two halves.
         auto extract_round = [&](uint32_t z, uint32_t xb, uint32_t sb, bool may_split) {
+            // prefix sum of the per-lane counts (0..8) from four ballots: the bits of the counts are summed
+            // by population counts, all independent -- a shuffle scan is five dependent round trips
             const uint32_t cnt = __popc(z);
-            uint32_t incl = cnt;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-                if (lane >= d) incl += t;
-            }
-            const uint32_t tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+            const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, cnt & 1u), b1 = __ballot_sync(0xFFFFFFFFu, cnt & 2u);
+            const uint32_t b2 = __ballot_sync(0xFFFFFFFFu, cnt & 4u), b3 = __ballot_sync(0xFFFFFFFFu, cnt & 8u);
+            const uint32_t tot = __popc(b0) + 2u * __popc(b1) + 4u * __popc(b2) + 8u * __popc(b3);
             if (may_split && tot > 128u) return false;
-            uint2* dst = q1 + n1 + (incl - cnt);
-            while (z) {
-                const uint32_t bit = 31u - (uint32_t)__clz(z);
-                z ^= 1u << bit;
-                *dst++ = make_uint2(xb + bit, sb + bit);
+            const uint32_t excl = __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt) + 8u * __popc(b3 & lt);
+            uint2* dst = q1 + n1 + excl;
+            while (z) {  // two survivors per trip: the highest and the lowest set bit
+                const uint32_t hi = 31u - (uint32_t)__clz(z), lo = (uint32_t)__ffs((int)z) - 1u;
+                dst[0] = make_uint2(xb + hi, sb + hi);
+                if (hi != lo) dst[1] = make_uint2(xb + lo, sb + lo);
+                dst += 2;  // (a lone last survivor leaves dst one too far: it is not used again)
+                z &= ~((1u << hi) | (1u << lo));
             }
             __syncwarp();
             n1 += tot;
@@ -561,7 +562,7 @@ inline int lean_plan(int fmt, uint32_t L, uint32_t B, LeanPlan* p)
     p->RC = 4 * p->R;
     p->n_steps_total = (L / 4) / p->R;
     // (Two CTAs per SM fit the bit-packed ring, but need <= 60 registers per thread: the spills cost
-    // more than the second CTA hides -- 46 against 40 us per phase, profiles/r2_lean_notes.md.)
+    // more than the second CTA hides -- 46 against 40 us per phase, DESIGN.md appendix B.)
     p->nb = p->n_steps_total < per_lat ? p->n_steps_total : per_lat;
     const uint32_t avail = (uint32_t)smem_optin - 256 - kLeanFixedBytes;
     const uint32_t chunk_bits_bytes = p->RC * p->pitch;

@@ -14,7 +14,7 @@
 //     the stencil code whose negative offsets get the ring size added.  (The
 //     alternative, PGG_RING_MIRROR=1, stages the three rows above slot 0 a second
 //     time in front of it -- no wrap at all, but 24 KB that a sixth ring slot
-//     uses better: 65.0 -> 63.5 us per launch, profiles/r1_ring_design_notes.md);
+//     uses better: 65.0 -> 63.5 us per launch, DESIGN.md appendix A);
 //   * queue entries are self-contained: Q1 = (soff, site), Q2 = (soff|dir|s_x,
 //     site, u); soff = offset of x from ring0 in site units (bytes for uint8,
 //     bits for bit-packed), site = lattice site index (the Philox counter and
@@ -62,7 +62,7 @@ constexpr int kRingQ2Cap = 64;    // 16-byte entries per warp (a ring: power of 
 constexpr int kRingMaxSlots = 6;
 // Q2 (a second compaction between the Philox draw and the stencil) fills its batches of 32
 // only half on average -- a site may wait for one step only -- and its 16 KB are worth more
-// as ring slots (profiles/r1_ring_design_notes.md), so level 2 runs inline under divergence.
+// as ring slots (DESIGN.md appendix A), so level 2 runs inline under divergence.
 // The bit-packed stencil (a shift and a mask per read) is dearer, there Q2 still pays.
 template <int FMT> struct RingCfg {
     static constexpr bool q2 = FMT == kFmtBits;
@@ -229,7 +229,7 @@ __device__ __forceinline__ RingDraw ring_draw(uint2 e, const uint8_t* ring0, con
 // FR ("full row", implies FULL): one strip = the whole lattice row, staged without halo columns,
 // so the rows of a chunk are contiguous in global AND shared memory and arrive as ONE bulk copy
 // (rows of 512 B ... 8 KB copied singly stream at a fraction of the rate, profiles/
-// r1_ring_design_notes.md); the periodic column wrap is resolved in the few sites near a row end.
+// DESIGN.md appendix A); the periodic column wrap is resolved in the few sites near a row end.
 template <int FMT, bool FULL, bool FR>
 __global__ void __launch_bounds__(kRingThreads, 1)
 phase_ring_kernel(PhaseArgs a, uint32_t m, uint32_t k, RingPlan g)
@@ -641,7 +641,7 @@ inline int ring_plan(int fmt, uint32_t L, uint32_t B, RingPlan* p, bool allow_fu
     if (const char* e = getenv("PGG_RING_MIRROR")) p->mirror = (atoi(e) && !p->fullrow) ? 1u : 0u;
     p->rotate = 1;
     if (const char* e = getenv("PGG_RING_ROTATE")) p->rotate = atoi(e) ? 1u : 0u;
-    p->l2pf = 3;  // chunks; measured: 58.6 -> 58.1 us per launch (profiles/r1_ring_design_notes.md)
+    p->l2pf = 3;  // chunks; measured: 58.6 -> 58.1 us per launch (DESIGN.md appendix A)
     if (const char* e = getenv("PGG_RING_L2PF")) p->l2pf = (uint32_t)std::max(0, std::min(64, atoi(e)));
     const uint32_t fixed = (uint32_t)(fmt == kFmtU8 ? RingCfg<kFmtU8>::fixed_bytes : RingCfg<kFmtBits>::fixed_bytes)
                          + (p->mirror ? 3 * p->pitch : 0);

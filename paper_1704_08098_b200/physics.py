@@ -44,11 +44,11 @@ def window_stats(counts, sites, n_batches=10):
     return float(w.mean()), float(b.std(ddof=1) / math.sqrt(n_batches))
 
 
-def stationary(rs, seeds, L=400, n_mcs=20000, K=0.5, rho0=0.5, order=ORDER_IID):
+def stationary(rs, seeds, L=400, n_mcs=20000, K=0.5, rho0=0.5, order=ORDER_IID, fmt=FMT_U8):
     """-> {r: {"per_seed": [(mean, stderr)...], "mean": m, "stderr": e}}; e combines the batch-mean
     errors with the scatter between seeds (whichever is larger)."""
     pairs = [(r, s) for r in rs for s in seeds]
-    tr = run_traces(L, [p[0] for p in pairs], [p[1] for p in pairs], K, rho0, n_mcs, order)
+    tr = run_traces(L, [p[0] for p in pairs], [p[1] for p in pairs], K, rho0, n_mcs, order, fmt)
     out = {}
     for a, r in enumerate(rs):
         st = [window_stats(tr[a * len(seeds) + b], L * L) for b in range(len(seeds))]
@@ -146,7 +146,7 @@ def main():
     ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"])
     ap.add_argument("--rs", type=float, nargs="+", default=None)
     ap.add_argument("--r", type=float, default=3.7443)
-    ap.add_argument("--fmt", default="u8", choices=["u8", "bits"], help="lattice layout (decay only; same trajectories)")
+    ap.add_argument("--fmt", default="u8", choices=["u8", "bits"], help="lattice layout (same trajectories; bits is the fast path for L >= 1024)")
     args = ap.parse_args()
     order = {"iid": ORDER_IID, "perm": ORDER_PERM, "dtile": ORDER_DTILE}[args.order]
     if args.what == "fig5":
@@ -154,9 +154,11 @@ def main():
                           "rows": fig5(order, args.mcs or 2000)}))
     elif args.what == "stationary":
         rs = args.rs or [round(3.60 + 0.05 * a, 2) for a in range(9)] + [5.3, 5.4, 5.5, 5.6]
-        res = stationary(rs, args.seeds or [101, 102, 103, 104], args.L or 400, args.mcs or 20000, order=order)
+        seeds = args.seeds or [101, 102, 103, 104]
+        res = stationary(rs, seeds, args.L or 400, args.mcs or 20000, order=order,
+                         fmt=FMT_BITS if args.fmt == "bits" else FMT_U8)
         print(json.dumps({"what": "stationary", "order": args.order, "L": args.L or 400, "mcs": args.mcs or 20000,
-                          "rows": [{"r": r, **v} for r, v in res.items()]}))
+                          "fmt": args.fmt, "seeds": seeds, "rows": [{"r": r, **v} for r, v in res.items()]}))
     else:
         seeds = args.seeds or list(range(1, 17))
         rows = decay(args.r, seeds, args.L or 2048, args.mcs or 100000, order=order,
