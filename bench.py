@@ -178,7 +178,7 @@ def run_ours(args):
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
                "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND,
-               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT, "lean": pgg.VARIANT_LEAN, "persist": pgg.VARIANT_PERSIST}[args.variant]
+               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT, "lean": pgg.VARIANT_LEAN, "persist": pgg.VARIANT_PERSIST, "cluster": pgg.VARIANT_CLUSTER}[args.variant]
     pgg.pgg_set_variant(variant)
     seed = SEED + rank
     shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
@@ -394,7 +394,7 @@ def main():
     ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
-    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "pipe", "band", "ring", "split", "dyn", "resident", "lean", "persist"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "pipe", "band", "ring", "split", "dyn", "resident", "lean", "persist", "cluster"])
     ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"],
                     help="schedule: the 16-sublattice schedule with i.i.d. (bench default) or permuted classes, or "
                          "the paper's own double-tiling schedule (PAPER.md:75-93); anything but iid is not the bench workload")

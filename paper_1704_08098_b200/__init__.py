@@ -23,7 +23,7 @@ FMT_U8, FMT_BITS = 0, 1
 ORDER_IID, ORDER_PERM, ORDER_DTILE = 0, 1, 2
 VARIANT_AUTO, VARIANT_V0, VARIANT_TILE = 0, 1, 2
 VARIANT_PIPE, VARIANT_BAND, VARIANT_RING, VARIANT_SPLIT, VARIANT_DYN, VARIANT_RESIDENT = 4, 5, 6, 7, 8, 9
-VARIANT_DTILE, VARIANT_LEAN, VARIANT_PERSIST = 10, 11, 12
+VARIANT_DTILE, VARIANT_LEAN, VARIANT_PERSIST, VARIANT_CLUSTER = 10, 11, 12, 13
 
 # name -> (restype, argtypes); also the list of symbols include/pgg.h declares
 _u32p, _u64p, _u8p, _f64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_uint8),

@@ -23,6 +23,7 @@
 #include "pgg_kernels_dyn.cuh"
 #include "pgg_kernels_resident.cuh"
 #include "pgg_kernels_lean.cuh"
+#include "pgg_kernels_cluster.cuh"
 #include "pgg_kernels_dtile.cuh"
 #include "pgg_kernels_probe.cuh"
 
@@ -195,9 +196,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     }
     if (pd) {  // two kernels carry the second game: LEAN where it runs, else the general V0
         const int asked = g_variant.load();
-        if (asked != PGG_VARIANT_AUTO && asked != PGG_VARIANT_V0 && asked != PGG_VARIANT_LEAN && asked != PGG_VARIANT_PERSIST)
-            return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs on variants V0, LEAN and PERSIST only (asked: %d)", asked);
+        if (asked != PGG_VARIANT_AUTO && asked != PGG_VARIANT_V0 && asked != PGG_VARIANT_LEAN && asked != PGG_VARIANT_PERSIST &&
+            asked != PGG_VARIANT_CLUSTER)
+            return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs on variants V0, LEAN, PERSIST and CLUSTER only (asked: %d)", asked);
         variant = asked == PGG_VARIANT_PERSIST ? PGG_VARIANT_PERSIST
+                : asked == PGG_VARIANT_CLUSTER ? PGG_VARIANT_CLUSTER
                 : (asked != PGG_VARIANT_V0 && pgg::lean_supported(fmt, L)) ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;
         if (asked == PGG_VARIANT_LEAN && variant != PGG_VARIANT_LEAN)
             return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", asked, fmt, L);
@@ -205,6 +208,8 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     if (variant == PGG_VARIANT_RESIDENT && !res_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_LEAN && !pgg::lean_supported(fmt, L))
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
+    if (variant == PGG_VARIANT_CLUSTER && !pgg::cluster_supported(fmt, L))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_PERSIST && !pgg::lean_persist_supported(fmt, L, B))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u, B %u", variant, fmt, L, B);
@@ -315,6 +320,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     }
 
     pgg::LeanPlan lplan;
+    pgg::ClusterPlan cplan;
+    if (variant == PGG_VARIANT_CLUSTER) {
+        int32_t rc = pgg::cluster_plan(fmt, L, &cplan);
+        if (rc != 0) return fail(PGG_ERR_CUDA, "cluster kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
+    }
     unsigned int* d_gbar = nullptr;
     if (variant == PGG_VARIANT_PERSIST) {
         PGG_CUDA(tmp.alloc((void**)&d_gbar, sizeof(unsigned int) * B));
@@ -335,6 +345,11 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         PGG_LAUNCHED();
         if (variant == PGG_VARIANT_RESIDENT) {  // all 16 * n_chunk phases in one launch
             pgg::resident_launch(resplan, fmt, a, m0, n_chunk, B, stream);
+            PGG_LAUNCHED();
+            continue;
+        }
+        if (variant == PGG_VARIANT_CLUSTER) {   // likewise; the lattice stays in the cluster's shared memory
+            PGG_CUDA(pgg::cluster_launch(cplan, fmt, a, m0, n_chunk, B, stream, game));
             PGG_LAUNCHED();
             continue;
         }
@@ -510,7 +525,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_PERSIST || variant == PGG_VARIANT_DTILE || variant == 3)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_CLUSTER || variant == PGG_VARIANT_DTILE || variant == 3)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -531,6 +546,7 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_RESIDENT) return pgg::resident_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_LEAN) return pgg::lean_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_PERSIST) return pgg::lean_persist_supported(fmt, L, 1) ? 1 : 0;
+    if (variant == PGG_VARIANT_CLUSTER) return pgg::cluster_supported(fmt, L) ? 1 : 0;
     return 0;
 }
 

@@ -410,6 +410,8 @@ LONG_CASES = [
     ("LEAN", pgg.FMT_U8, 1024, {}),                              # LEAN, uint8 packed to bits on chip
     ("LEAN", pgg.FMT_BITS, 1024, {}),                            # LEAN, bit-packed source
     ("PERSIST", pgg.FMT_BITS, 1024, {}),                         # LEAN, one cooperative launch per 4096 MCS
+    ("CLUSTER", pgg.FMT_U8, 1024, {}),                           # lattice resident in a cluster's shared memory
+    ("CLUSTER", pgg.FMT_BITS, 1024, {}),
 ]
 
 
@@ -438,7 +440,7 @@ def test_one_call_longer_than_an_order_chunk(name, fmt, L, env, monkeypatch):
 
 
 @pytest.mark.parametrize("name,fmt,L,env", LONG_CASES,
-                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits", "PERSIST-bits"])
+                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits", "PERSIST-bits", "CLUSTER-u8", "CLUSTER-bits"])
 @pytest.mark.parametrize("t0", [99900, 2**32 - 40])
 def test_streaming_kernels_late_windows(name, fmt, L, env, t0, monkeypatch):
     """SURVEY 8(d) late windows (t = 99 900) and the counter width (t_begin + m up to 2^32 - 1)
@@ -572,6 +574,54 @@ def test_persist_ensemble_equals_oracle():
     torch.cuda.synchronize()
     got = to_host(d, fmt, L)
     for b in (0, 7, 15):
+        ref = orc.init(L, 0.5, seeds[b])
+        ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs, n_threads=orc.max_threads())
+        assert_same(got[b], ref, f"member {b}")
+        assert_same(cnt[b].cpu().numpy().astype(np.uint64), ref_counts)
+
+
+# ---------------------------------------------------------------- CLUSTER (lattice resident in a CTA cluster)
+@pytest.mark.parametrize("fmt", FMTS)
+@pytest.mark.parametrize("L,n_mcs", [(1024, 8), (2048, 5), (4096, 3)])
+def test_cluster_parity_sizes(fmt, L, n_mcs):
+    """The lattice stays in the shared memory of 8 (L = 4096: 16) CTAs for the whole call; halo rows travel
+    over distributed shared memory after every phase.  Lattice and counts against the oracle; one sweep
+    launch per call; dense and sparse starts, both orders, a 64-bit seed, a late t_begin."""
+    use_variant(pgg.VARIANT_CLUSTER, fmt, L)
+    for seed, r, order, rho0, t0 in ((L + 1, 3.8, pgg.ORDER_IID, 0.5, 3), (2**35 + L, 4.6, pgg.ORDER_PERM, 0.1, 2**32 - 20)):
+        lat0 = orc.init(L, rho0, seed)
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, r, K, seed, order, t0, n_mcs, n_threads=orc.max_threads())
+        before = pgg.pgg_launch_count()
+        got, counts = gpu_sweep(lat0, fmt, r, seed, order, t0, n_mcs)
+        assert pgg.pgg_get_variant_used() == pgg.VARIANT_CLUSTER
+        assert pgg.pgg_launch_count() - before == 5       # upload, density, order, ONE sweep launch, finalize
+        assert_same(got, ref, f"lattice L={L}")
+        assert_same(counts, ref_counts, f"counts L={L}")
+
+
+@pytest.mark.parametrize("fmt", FMTS)
+def test_cluster_structured_ensembles_and_waves(fmt):
+    """Structured and absorbing states; an ensemble of 40 lattices of L = 1024 (more clusters than the GPU
+    holds at once: they run in waves); members against the oracle."""
+    L = 1024
+    use_variant(pgg.VARIANT_CLUSTER, fmt, L)
+    for n, lat0 in enumerate([wl.checkerboard_lattice(L), wl.stripes_lattice(L, 7, False), wl.blobs_lattice(L, 3),
+                              np.zeros((L, L), np.uint8), np.ones((L, L), np.uint8)]):
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, 3.8, K, 70 + n, pgg.ORDER_IID, 0, 4, n_threads=orc.max_threads())
+        got, counts = gpu_sweep(lat0, fmt, 3.8, 70 + n, pgg.ORDER_IID, 0, 4)
+        assert_same(got, ref, f"state {n}")
+        assert_same(counts, ref_counts, f"counts state {n}")
+    B, n_mcs = 40, 3
+    rs = [3.7 + 0.005 * b for b in range(B)]
+    seeds = [2**33 + 3 * b for b in range(B)]
+    d = empty_lattice(fmt, L, B)
+    cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, n_mcs, cnt)
+    torch.cuda.synchronize()
+    got = to_host(d, fmt, L)
+    for b in (0, 17, 39):
         ref = orc.init(L, 0.5, seeds[b])
         ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs, n_threads=orc.max_threads())
         assert_same(got[b], ref, f"member {b}")
