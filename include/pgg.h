@@ -100,9 +100,9 @@ enum {
                                 bits on arrival (uint8), scan / draw / stencil on a bit ring   */
     PGG_VARIANT_PERSIST = 12,/* LEAN, bit-packed, <= 148 lattices: every phase of up to 4096 MCS in ONE
                                 cooperative launch, a per-lattice barrier between phases           */
-    PGG_VARIANT_CLUSTER = 13 /* L = 1024, 2048, 4096, both layouts: the lattice stays bit-packed in the shared
-                                memory of a CTA cluster (8 or 16 CTAs) for the whole call, halo rows over
-                                distributed shared memory, one cluster barrier per phase              */
+    PGG_VARIANT_CLUSTER = 13 /* L = 128 .. 4096 (a power of two), both layouts: the lattice stays bit-packed in
+                                the shared memory of a CTA cluster (1 .. 16 CTAs) for the whole call, halo rows
+                                over distributed shared memory, one cluster barrier per phase          */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:

@@ -189,7 +189,13 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         // bit-packed: LEAN (rows stream into a bit ring, queue lifetime of several steps) measured 2-3x
         // faster than BAND on ensembles and sparse states and level with it on the dense C5 lattice
         const bool lean_bits = fmt == PGG_FMT_BITS && pgg::lean_supported(fmt, L);
-        variant = (res_ok && res_pays) ? PGG_VARIANT_RESIDENT
+        // CLUSTER (the lattice resident in a CTA cluster's shared memory for the whole call; appendix B):
+        // L = 512: 2.3-3.6 us per phase against RESIDENT's 5.3-6.9 and RING's 4.2-9.2 at every batch size;
+        // L = 1024: 2.8 against 4.3 for one lattice, 8.7 against 11.9 for 64; L = 2048 from 32 lattices
+        // (28.7 against 33 / 52 at 64); never at L = 4096 (16 CTAs per lattice leave the GPU idle)
+        const bool cluster_pays = pgg::cluster_supported(fmt, L) && (L == 512 || L == 1024 || (L == 2048 && B >= 32));
+        variant = cluster_pays ? PGG_VARIANT_CLUSTER
+                : (res_ok && res_pays) ? PGG_VARIANT_RESIDENT
                 : lean_bits ? PGG_VARIANT_LEAN
                 : !stream_pays ? PGG_VARIANT_V0
                 : (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
@@ -201,6 +207,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
             return fail(PGG_ERR_UNSUPPORTED, "the prisoner's dilemma runs on variants V0, LEAN, PERSIST and CLUSTER only (asked: %d)", asked);
         variant = asked == PGG_VARIANT_PERSIST ? PGG_VARIANT_PERSIST
                 : asked == PGG_VARIANT_CLUSTER ? PGG_VARIANT_CLUSTER
+                : (asked == PGG_VARIANT_AUTO && (L == 512 || L == 1024)) ? PGG_VARIANT_CLUSTER
                 : (asked != PGG_VARIANT_V0 && pgg::lean_supported(fmt, L)) ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;
         if (asked == PGG_VARIANT_LEAN && variant != PGG_VARIANT_LEAN)
             return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", asked, fmt, L);
@@ -322,7 +329,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     pgg::LeanPlan lplan;
     pgg::ClusterPlan cplan;
     if (variant == PGG_VARIANT_CLUSTER) {
-        int32_t rc = pgg::cluster_plan(fmt, L, &cplan);
+        int32_t rc = pgg::cluster_plan(fmt, L, B, &cplan);
         if (rc != 0) return fail(PGG_ERR_CUDA, "cluster kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
     }
     unsigned int* d_gbar = nullptr;

@@ -1,4 +1,4 @@
-// pgg_kernels_cluster.cuh -- the CLUSTER kernel: one lattice of L = 1024 .. 4096 stays BIT-PACKED in
+// pgg_kernels_cluster.cuh -- the CLUSTER kernel: one lattice of L = 128 .. 4096 (a power of two) stays BIT-PACKED in
 // the shared memory of a thread-block cluster for a whole call ("minimizing
 // the need to access global memory, and to make full use of the registers and the shared memory").
 //
@@ -7,7 +7,7 @@
 // -- and neither fewer bytes (LEAN) nor fewer launches (PERSIST) shorten that chain.  Keeping the rows
 // on chip does: nothing is staged, nothing waits for a copy, and the queues are drained once per phase.
 //
-//   cluster  = CS CTAs (8; 16 for L = 4096, a non-portable size) = one lattice; grid = (CS, B)
+//   cluster  = CS CTAs (1 .. 16, from L and the number of lattices; 16 is a non-portable size) = one lattice; grid = (CS, B)
 //   band     = the L/CS consecutive rows CTA `rank` owns, plus three halo rows above and below, all in
 //              its shared memory as bits (uint8 lattices are packed on load and unpacked on store:
 //              the layout in HBM is the caller's, the layout on chip is ours)
@@ -42,7 +42,7 @@ struct ClusterPlan {
     uint32_t lgWPR;    // log2(words per row)
     uint32_t CS;       // CTAs per cluster = bands per lattice
     uint32_t rows;     // rows per band = L / CS (a multiple of 4)
-    uint32_t words_per_phase;  // (rows / 4) * (L / 32): a multiple of 512
+    uint32_t words_per_phase;  // (rows / 4) * (L / 32): a multiple of 32 (whole warps)
     uint32_t smem_bytes;
 };
 
@@ -280,32 +280,73 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
 // ---------------------------------------------------------------------------
 inline bool cluster_supported(int /*fmt*/, uint32_t L)
 {
-    return L == 1024 || L == 2048 || L == 4096;
+    return L >= 128 && L <= 4096 && (L & (L - 1)) == 0;  // whole 32-site words, power-of-two rows, fits 16 CTAs
 }
 
-inline int cluster_plan(int fmt, uint32_t L, ClusterPlan* p)
+inline int cluster_plan(int fmt, uint32_t L, uint32_t B, ClusterPlan* p)
 {
     uint32_t lg = 0;
     while ((1u << lg) < L) ++lg;
     p->lg2L = lg;
     p->pitch = L / 8;
     p->lgWPR = lg - 5;
-    p->CS = L == 4096 ? 16u : 8u;
-    if (const char* s = getenv("PGG_CLUSTER_SIZE")) {
-        const uint32_t v = (uint32_t)atoi(s);
-        if ((v == 2 || v == 4 || v == 8 || v == 16) && (L / v) % 4 == 0 && ((L / v / 4) * (L / 32)) % 512 == 0) p->CS = v;
-    }
-    p->rows = L / p->CS;
-    p->words_per_phase = (p->rows / 4) * (L / 32);
-    p->smem_bytes = (p->rows + 6) * p->pitch + kClusterFixedBytes;
-    const void* kernels[4] = {(const void*)sweep_cluster_kernel<kFmtU8, kGamePGG>, (const void*)sweep_cluster_kernel<kFmtBits, kGamePGG>,
-                              (const void*)sweep_cluster_kernel<kFmtU8, kGamePD>, (const void*)sweep_cluster_kernel<kFmtBits, kGamePD>};
-    int dev = 0, smem_optin = 0;
+    int dev = 0, smem_optin = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return (int)e;
     e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     if (e != cudaSuccess) return (int)e;
-    if (p->smem_bytes > (uint32_t)smem_optin) return (int)cudaErrorInvalidValue;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return (int)e;
+    // CTAs per lattice.  Measured (DESIGN.md appendix B): a phase costs ~1.7 us + ~1.1 us per round of 512
+    // words, so a lattice wants as many CTAs as give it half a round each -- as long as every lattice's
+    // cluster is resident at once (the occupancy query knows how many clusters of a size the GPCs hold);
+    // a larger ensemble takes the smallest cluster that fits shared memory and runs in waves.
+    auto fits = [&](uint32_t cs) { return (L / cs) % 4 == 0 && (L / cs + 6) * p->pitch + (uint32_t)kClusterFixedBytes <= (uint32_t)smem_optin; };
+    const void* k0 = fmt == kFmtU8 ? (const void*)sweep_cluster_kernel<kFmtU8, kGamePGG> : (const void*)sweep_cluster_kernel<kFmtBits, kGamePGG>;
+    cudaFuncSetAttribute(k0, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    auto resident = [&](uint32_t cs) -> uint32_t {   // clusters of size cs the device holds at once
+        const uint32_t smem = (L / cs + 6) * p->pitch + (uint32_t)kClusterFixedBytes;
+        if (cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(cs, B);
+        cfg.blockDim = dim3(kClusterThreads);
+        cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = cs;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, k0, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+        return (uint32_t)n;
+    };
+    uint32_t cs_max = 2 * (L / 128) * (L / 512);   // half a round per CTA: 2 L^2 / 65536
+    if (cs_max < 1) cs_max = 1;
+    if (cs_max > 16) cs_max = 16;
+    // cost model: waves x (1.7 us + 1.1 us per round); ties go to the smaller cluster
+    uint32_t cs = 0;
+    double best = 0.0;
+    for (uint32_t c = 1; c <= cs_max; c <<= 1) {
+        if (!fits(c)) continue;
+        const uint32_t res = resident(c);
+        if (res == 0) continue;
+        const double rounds = (double)L * L / (65536.0 * c);
+        const double cost = (double)((B + res - 1) / res) * (1.7 + 1.1 * (rounds < 0.5 ? 0.5 : rounds));
+        if (cs == 0 || cost < 0.97 * best) { cs = c; best = cost; }
+    }
+    if (const char* s = getenv("PGG_CLUSTER_SIZE")) {
+        const uint32_t v = (uint32_t)atoi(s);
+        if ((v == 1 || v == 2 || v == 4 || v == 8 || v == 16) && fits(v)) cs = v;
+    }
+    if (cs == 0) return (int)cudaErrorInvalidValue;
+    p->CS = cs;
+    p->rows = L / p->CS;
+    p->words_per_phase = (p->rows / 4) * (L / 32);   // a multiple of 32: whole warps
+    p->smem_bytes = (p->rows + 6) * p->pitch + kClusterFixedBytes;
+    const void* kernels[4] = {(const void*)sweep_cluster_kernel<kFmtU8, kGamePGG>, (const void*)sweep_cluster_kernel<kFmtBits, kGamePGG>,
+                              (const void*)sweep_cluster_kernel<kFmtU8, kGamePD>, (const void*)sweep_cluster_kernel<kFmtBits, kGamePD>};
     for (const void* kern : kernels) {
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes);
         if (e != cudaSuccess) return (int)e;

@@ -12,7 +12,7 @@ ROOT = Path(__file__).resolve().parents[1]
 
 
 def run_bench(*extra):
-    cmd = [sys.executable, str(ROOT / "bench.py"), "--L", "1024", "--mcs", "20", "--steps", "2", "--warmup", "3", *extra]
+    cmd = [sys.executable, str(ROOT / "bench.py"), "--L", "2048", "--mcs", "20", "--steps", "2", "--warmup", "3", *extra]
     p = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert p.returncode == 0, p.stderr[-2000:]
     lines = [ln for ln in p.stdout.splitlines() if ln.startswith("{")]
@@ -29,7 +29,7 @@ def test_bench_line_has_the_contract_keys():
     assert d["dtype"] == "u8" and d["data"] == "synthetic" and d["vs_baseline"] is None
     assert "workload" in d["config"] and "model" not in d["config"]
     assert d["value"] > 0 and d["e2e"]["value"] > 0
-    assert d["e2e"]["h2d_bytes_per_step"] == 1024 * 1024 and d["e2e"]["d2h_bytes_per_step"] > 1024 * 1024
+    assert d["e2e"]["h2d_bytes_per_step"] == 2048 * 2048 and d["e2e"]["d2h_bytes_per_step"] > 2048 * 2048
     # (seed upload + init) + (seed/table upload + density + order + 16 phases per MCS + finalize), per step
     assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 1 + 16 * 20 + 1))
     r = d["roofline"]
@@ -58,7 +58,7 @@ def test_bench_line_for_the_papers_schedule():
     assert d["config"]["order_mode"] == "dtile" and d["config"]["variant"] == 10
     assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 4 * 20 + 1))
     r = d["roofline"]
-    assert r["algorithmic_bytes_per_launch"] == 1024 * 1024 * 1.25 and "dtile_part_kernel" in r["kernel"]
+    assert r["algorithmic_bytes_per_launch"] == 2048 * 2048 * 1.25 and "dtile_part_kernel" in r["kernel"]
     assert d["value"] > 0 and d["e2e"]["value"] > 0 and 0.0 <= d["final_rho_C"] <= 1.0
 
 
@@ -67,6 +67,6 @@ def test_bench_line_for_the_bit_packed_layout():
     second against the Philox-only ceiling) with the HBM view kept as context."""
     d = run_bench("--fmt", "bits", "--no-cpu-baseline")
     r = d["roofline"]
-    assert d["dtype"].startswith("u1") and d["config"]["variant"] == 11      # AUTO -> LEAN
+    assert d["dtype"].startswith("u1") and d["config"]["variant"] == 11      # AUTO -> LEAN at L = 2048, one lattice
     assert r["bound"] == "alu" and r["unit"] == "Gdraw/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
-    assert 0.0 < r["draw_fraction"] <= 1.0 and r["hbm_context"]["algorithmic_bytes_per_launch"] == 1024 * 1024 * 17 / 16 / 8
+    assert 0.0 < r["draw_fraction"] <= 1.0 and r["hbm_context"]["algorithmic_bytes_per_launch"] == 2048 * 2048 * 17 / 16 / 8

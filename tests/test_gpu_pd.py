@@ -57,7 +57,7 @@ def test_pd_parity_v0_sizes(fmt, L):
 @pytest.mark.parametrize("fmt", [pgg.FMT_U8, pgg.FMT_BITS])
 @pytest.mark.parametrize("L,n_mcs", [(1024, 12), (2048, 6), (4096, 3)])
 def test_pd_parity_lean(fmt, L, n_mcs):
-    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    pgg.pgg_set_variant(pgg.VARIANT_LEAN)
     for seed, pay, K, order, t0 in ((L + 3, WEAK, 0.1, pgg.ORDER_IID, 0), (2**34 + L, GEN, 0.5, pgg.ORDER_PERM, 2**32 - 20)):
         lat0 = orc.init(L, 0.5, seed)
         ref = lat0.copy()
@@ -70,6 +70,22 @@ def test_pd_parity_lean(fmt, L, n_mcs):
     pgg.pgg_set_variant(pgg.VARIANT_V0)
     got_v0, counts_v0 = gpu_pd(lat0, fmt, pay, K, seed, order, t0, n_mcs)
     assert_same(got_v0, ref) and assert_same(counts_v0, ref_counts)
+
+
+@pytest.mark.parametrize("fmt", [pgg.FMT_U8, pgg.FMT_BITS])
+@pytest.mark.parametrize("L,n_mcs", [(512, 12), (1024, 8), (2048, 4)])
+def test_pd_parity_cluster(fmt, L, n_mcs):
+    """The cluster-resident kernel (AUTO's choice for L = 512 and 1024) with the pair-game payoffs."""
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO if L <= 1024 else pgg.VARIANT_CLUSTER)
+    for seed, pay, K, order, t0 in ((L + 5, WEAK, 0.1, pgg.ORDER_IID, 0), (2**34 + L, GEN, 0.5, pgg.ORDER_PERM, 2**32 - 20)):
+        lat0 = orc.init(L, 0.5, seed)
+        ref = lat0.copy()
+        ref_counts = orc.pd_sweep(ref, *pay, K, seed, order, t0, n_mcs)
+        got, counts = gpu_pd(lat0, fmt, pay, K, seed, order, t0, n_mcs)
+        assert pgg.pgg_get_variant_used() == pgg.VARIANT_CLUSTER
+        assert_same(got, ref, f"PD lattice L={L}")
+        assert_same(counts, ref_counts, f"PD counts L={L}")
+    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
 
 
 @pytest.mark.parametrize("fmt", [pgg.FMT_U8, pgg.FMT_BITS])
