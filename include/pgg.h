@@ -77,11 +77,15 @@ enum { PGG_FMT_U8 = 0, PGG_FMT_BITS = 1 };
  *   s_x != s_y and u < T[...] as in every mode.  Kernel variants do not apply. */
 enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
 
-/* Kernel variants of the phase step (all bit-identical; see DESIGN.md).
- * PGG_VARIANT_AUTO picks by measurement (DESIGN.md appendix B, DESIGN.md appendix B):
- * RESIDENT for L <= 320, and for L <= 512 from 3 lattices (6 at L = 512; uint8 L = 512: from 20, RING
- * below that); LEAN for the bit-packed layout at L = 1024 .. 32768 (powers of two); RING (uint8) / BAND
- * (bit-packed) for the other L >= 2048 and for uint8 L = 512, 1024; else V0.                          */
+/* Kernel variants of the phase step (all bit-identical; see DESIGN.md section 5).
+ * PGG_VARIANT_AUTO picks by measurement (DESIGN.md appendix B): CLUSTER for L = 512 and 1024 and for
+ * L = 2048 from 32 lattices; else RESIDENT for L <= 320 and for L <= 448 from 3 lattices; else LEAN for the
+ * bit-packed layout at L = 1024 .. 32768 (powers of two); else RING (uint8) / BAND (bit-packed) for
+ * L >= 2048 and for uint8 L = 512; else V0.  TILE, PIPE, SPLIT, DYN, BAND (uint8), PERSIST are rungs of the
+ * ladder kept for comparison: selectable, tested, never chosen.  Tuning knobs read from the environment by
+ * the plan functions (defaults are the measured best; every setting is bit-exact): PGG_PDL,
+ * PGG_RING_{SLOTS,L2PF,FULLROW,TPR_LOG2,MIRROR,ROTATE}, PGG_BAND_SLOTS, PGG_DYN_WARPS, PGG_PIPE_STAGES,
+ * PGG_TILE_{CTAS_PER_SM,STAGES}, PGG_LEAN_{LAG,AHEAD,SLOT_ROWS,SLOTS,WORDS}, PGG_CLUSTER_SIZE.            */
 enum {
     PGG_VARIANT_AUTO = 0,
     PGG_VARIANT_V0 = 1,   /* one thread per active site, global loads, any L % 4 == 0 */

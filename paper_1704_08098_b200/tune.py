@@ -62,7 +62,7 @@ def table(cases, variants):
 
 def main():
     what = sys.argv[1] if len(sys.argv) > 1 else "small"
-    variants = [VARIANT_V0, VARIANT_RESIDENT, VARIANT_RING, VARIANT_BAND, VARIANT_LEAN]
+    variants = [VARIANT_V0, VARIANT_RESIDENT, VARIANT_RING, VARIANT_BAND, VARIANT_LEAN, VARIANT_CLUSTER]
     if what == "small":
         cases = [(fmt, B, L, 3.8, 60, 300 if L <= 512 else 100)
                  for fmt in (FMT_U8, FMT_BITS) for L in (128, 256, 320, 400, 448, 512, 1024, 2048) for B in (1, 4, 13, 52)]
