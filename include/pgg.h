@@ -140,6 +140,34 @@ int32_t pgg_sweep(void* d_lat, int32_t fmt, uint32_t L, double r, double K, uint
                   int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
                   void* stream);
 
+/* pgg_sweep for callers that may not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same operation, same arguments, same
+ * results bit for bit (the 16-phase schedule of pgg_sweep), but the
+ * temporaries of the sweep -- the seed, the 153-entry acceptance table (Eq. 3),
+ * the initial cooperator count and the phase-class order of every MCS of the call (16 bytes
+ * per MCS) -- live in ONE file-scope device array of PGG_STATIC_SCRATCH_BYTES (65 KB, held
+ * by every GPU that loads the library until the process exits) instead of the stream-ordered
+ * pool.  The call makes no cudaMalloc / cudaMallocAsync / cudaFree and calls no allocating
+ * library routine; the caller still owns d_lat and d_counts.
+ *   limit   : n_mcs <= PGG_STATIC_MAX_MCS (4096) per call, else PGG_ERR_BAD_PARAM (split a
+ *             longer run into several calls: (t_begin = a, n = b) then (a + b, c) equals
+ *             (a, b + c) bit for bit, as for pgg_sweep); PGG_ORDER_IID / PGG_ORDER_PERM only
+ *             (PGG_ORDER_DTILE -> PGG_ERR_UNSUPPORTED).
+ *   kernels : the one pgg_sweep would pick for a single lattice among CLUSTER, RESIDENT,
+ *             LEAN, RING and V0 (pgg_set_variant is honoured for these five; any other
+ *             selected variant -> PGG_ERR_UNSUPPORTED).
+ *   sharing : every call on a device uses the same array and finds the previous call's
+ *             contents in it; the call overwrites all it reads (and clears the one counter
+ *             that must start at zero) in stream order.  Two calls that OVERLAP on the GPU
+ *             (different streams without an event between them, or two host threads) race
+ *             on the array: serialise them.  Calls on one stream are safe back to back.
+ * Other errors as pgg_sweep.                                                         */
+#define PGG_STATIC_MAX_MCS 4096u
+#define PGG_STATIC_SCRATCH_BYTES (1024u + 16u * PGG_STATIC_MAX_MCS)
+int32_t pgg_sweep_static(void* d_lat, int32_t fmt, uint32_t L, double r, double K, uint64_t seed,
+                         int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
+                         void* stream);
+
 /* Cooperator count sum_x d_x (Eq. 4; rho_C = count / L^2).
  * d_count: device uint64, overwritten.                                           */
 int32_t pgg_density(const void* d_lat, int32_t fmt, uint32_t L, uint64_t* d_count, void* stream);

@@ -34,6 +34,8 @@ SIGNATURES = {
                                      C.c_void_p]),
     "pgg_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_double, C.c_double, C.c_uint64,
                               C.c_int32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]),
+    "pgg_sweep_static": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_double, C.c_double, C.c_uint64,
+                                     C.c_int32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]),
     "pgg_density": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_void_p, C.c_void_p]),
     "pgg_run_ensemble": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_uint32, _f64p, C.c_double,
                                      _u64p, C.c_int32, C.c_double, C.c_uint32, C.c_uint32, C.c_void_p,
@@ -107,6 +109,17 @@ def pgg_sweep(d_lat, fmt: int, L: int, r: float, K: float, seed: int, order_mode
               n_mcs: int, d_counts=None, stream=None) -> None:
     _check(lib().pgg_sweep(_ptr(d_lat), fmt, L, r, K, seed, order_mode, t_begin, n_mcs, _ptr(d_counts),
                            _stream(stream)))
+
+
+STATIC_MAX_MCS = 4096  # PGG_STATIC_MAX_MCS
+
+
+def pgg_sweep_static(d_lat, fmt: int, L: int, r: float, K: float, seed: int, order_mode: int, t_begin: int,
+                     n_mcs: int, d_counts=None, stream=None) -> None:
+    """pgg_sweep without any device allocation (temporaries in the library's static device array);
+    n_mcs <= STATIC_MAX_MCS per call, calls that overlap on the GPU race (include/pgg.h)."""
+    _check(lib().pgg_sweep_static(_ptr(d_lat), fmt, L, r, K, seed, order_mode, t_begin, n_mcs, _ptr(d_counts),
+                                  _stream(stream)))
 
 
 def pgg_density(d_lat, fmt: int, L: int, d_count, stream=None) -> None:

@@ -7,6 +7,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -406,9 +407,157 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     return PGG_OK;
 }
 
+// ---- pgg_sweep_static: the temporaries of a one-lattice sweep in a file-scope device array --------
+// Layout (bytes): [0, 8) seed | [8, 16) initial cooperator count | [256, 868) acceptance table |
+// [1024, 1024 + 16 * PGG_STATIC_MAX_MCS) phase-class order.  In HOST code the name below is a host-side
+// stand-in, not a device address: only the pointer cudaGetSymbolAddress returns may go to a kernel.
+constexpr size_t kStaticSeedOff = 0, kStaticCount0Off = 8, kStaticTableOff = 256, kStaticOrderOff = 1024;
+static_assert(kStaticTableOff + sizeof(uint32_t) * pgg::kTableSize <= kStaticOrderOff, "table overlaps the order");
+static __device__ __align__(256) unsigned char g_static_scratch[PGG_STATIC_SCRATCH_BYTES];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_ptr[kStaticMaxDevices] = {};  // per device, resolved once with that device current
+
+// Device address of g_static_scratch on the CURRENT device (no allocation: the array is part of the module).
+int32_t static_scratch(unsigned char** out)
+{
+    int dev = -1;
+    PGG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(PGG_ERR_UNSUPPORTED, "device ordinal %d: at most %d devices", dev, kStaticMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (g_static_ptr[dev] == nullptr) {
+        void* p = nullptr;
+        PGG_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (p == nullptr || (reinterpret_cast<uintptr_t>(p) & 255u) != 0)
+            return fail(PGG_ERR_CUDA, "cudaGetSymbolAddress returned %p for the static scratch", p);
+        g_static_ptr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_static_ptr[dev];
+    return PGG_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+int32_t pgg_sweep_static(void* d_lat, int32_t fmt, uint32_t L, double r, double K, uint64_t seed,
+                         int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts, void* stream_)
+{
+    int32_t rc = check_lattice_args(d_lat, fmt, L);
+    if (rc != PGG_OK) return rc;
+    if (order_mode == PGG_ORDER_DTILE)
+        return fail(PGG_ERR_UNSUPPORTED, "pgg_sweep_static runs the 16-sublattice schedule only (PGG_ORDER_IID / PGG_ORDER_PERM)");
+    if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM)
+        return fail(PGG_ERR_UNSUPPORTED, "unknown order_mode %d", order_mode);
+    if (!(K > 0.0) || !std::isfinite(K)) return fail(PGG_ERR_BAD_PARAM, "K must be finite and > 0");
+    if (!std::isfinite(r)) return fail(PGG_ERR_BAD_PARAM, "r is not finite");
+    if ((unsigned long long)t_begin + n_mcs > 4294967296ull)
+        return fail(PGG_ERR_BAD_PARAM, "t_begin + n_mcs exceeds 2^32");
+    if (n_mcs > PGG_STATIC_MAX_MCS)
+        return fail(PGG_ERR_BAD_PARAM, "n_mcs = %u exceeds PGG_STATIC_MAX_MCS = %u: the static scratch holds the class order "
+                    "of %u MCS; split the run into several calls", n_mcs, PGG_STATIC_MAX_MCS, PGG_STATIC_MAX_MCS);
+    if (n_mcs == 0) return PGG_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+
+    // the kernel pgg_sweep's AUTO rule picks for ONE lattice (run_sweeps above), among the five this entry point carries
+    int variant = g_variant.load();
+    if (variant == PGG_VARIANT_AUTO) {
+        const bool stream_pays = L >= 2048 || (fmt == PGG_FMT_U8 && L >= 512 && (L & (L - 1)) == 0);
+        variant = (pgg::cluster_supported(fmt, L) && (L == 512 || L == 1024)) ? PGG_VARIANT_CLUSTER
+                : (pgg::resident_supported(fmt, L) && L <= 320) ? PGG_VARIANT_RESIDENT
+                : (fmt == PGG_FMT_BITS && pgg::lean_supported(fmt, L)) ? PGG_VARIANT_LEAN
+                : (stream_pays && fmt == PGG_FMT_U8 && pgg::ring_supported(fmt, L)) ? PGG_VARIANT_RING : PGG_VARIANT_V0;
+    }
+    const bool ok = variant == PGG_VARIANT_V0 || (variant == PGG_VARIANT_CLUSTER && pgg::cluster_supported(fmt, L)) ||
+                    (variant == PGG_VARIANT_RESIDENT && pgg::resident_supported(fmt, L)) ||
+                    (variant == PGG_VARIANT_LEAN && pgg::lean_supported(fmt, L)) ||
+                    (variant == PGG_VARIANT_RING && pgg::ring_supported(fmt, L));
+    if (!ok) return fail(PGG_ERR_UNSUPPORTED, "pgg_sweep_static: variant %d is not available for fmt %d, L %u", variant, fmt, L);
+    g_variant_used = variant;
+
+    unsigned char* scratch = nullptr;
+    rc = static_scratch(&scratch);
+    if (rc != PGG_OK) return rc;
+    uint64_t* d_seed = reinterpret_cast<uint64_t*>(scratch + kStaticSeedOff);
+    unsigned long long* d_count0 = reinterpret_cast<unsigned long long*>(scratch + kStaticCount0Off);
+    uint32_t* d_table = reinterpret_cast<uint32_t*>(scratch + kStaticTableOff);
+    uint8_t* d_order = scratch + kStaticOrderOff;
+
+    uint32_t h_table[pgg::kTableSize];
+    rc = pgg_build_accept_table(r, K, h_table);
+    if (rc != PGG_OK) return rc;
+    rc = upload_params(1, &seed, h_table, d_seed, d_table, stream);  // kernel arguments: no staging buffer
+    if (rc != PGG_OK) return rc;
+
+    uint8_t* d_lats = static_cast<uint8_t*>(d_lat);
+    if (d_counts != nullptr) {
+        PGG_CUDA(cudaMemsetAsync(d_count0, 0, sizeof(unsigned long long), stream));  // the array keeps the last call's value
+        PGG_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(uint64_t) * (size_t)n_mcs, stream));
+        rc = launch_density(d_lats, fmt, 1, L, d_count0, 1, stream);
+        if (rc != PGG_OK) return rc;
+    }
+
+    pgg::PhaseArgs a;
+    a.lats = d_lats;
+    a.lat_bytes = lattice_bytes(fmt, L);
+    a.seeds = d_seed;
+    a.tables = d_table;
+    a.order = d_order;
+    a.deltas = reinterpret_cast<unsigned long long*>(d_counts);
+    a.L = L;
+    a.order_stride = n_mcs;
+    a.n_mcs = n_mcs;
+    a.t_begin = t_begin;
+
+    pgg::order_kernel<<<(n_mcs + 127) / 128, 128, 0, stream>>>(d_seed, 1, t_begin, n_mcs, n_mcs, order_mode, d_order);
+    PGG_LAUNCHED();
+    if (variant == PGG_VARIANT_RESIDENT) {
+        pgg::ResPlan plan;
+        int32_t e = pgg::resident_plan(fmt, L, &plan);
+        if (e != 0) return fail(PGG_ERR_CUDA, "resident kernel setup failed: %s", cudaGetErrorString((cudaError_t)e));
+        pgg::resident_launch(plan, fmt, a, 0, n_mcs, 1, stream);
+        PGG_LAUNCHED();
+    } else if (variant == PGG_VARIANT_CLUSTER) {
+        pgg::ClusterPlan plan;
+        int32_t e = pgg::cluster_plan(fmt, L, 1, &plan);
+        if (e != 0) return fail(PGG_ERR_CUDA, "cluster kernel setup failed: %s", cudaGetErrorString((cudaError_t)e));
+        PGG_CUDA(pgg::cluster_launch(plan, fmt, a, 0, n_mcs, 1, stream, pgg::kGamePGG));
+        PGG_LAUNCHED();
+    } else {
+        pgg::LeanPlan lplan;
+        pgg::RingPlan rplan;
+        if (variant == PGG_VARIANT_LEAN) {
+            int32_t e = pgg::lean_plan(fmt, L, 1, &lplan);
+            if (e != 0) return fail(PGG_ERR_CUDA, "lean kernel setup failed: %s", cudaGetErrorString((cudaError_t)e));
+        }
+        if (variant == PGG_VARIANT_RING) {
+            int32_t e = pgg::ring_plan(fmt, L, 1, &rplan);
+            if (e != 0) return fail(PGG_ERR_CUDA, "ring kernel setup failed: %s", cudaGetErrorString((cudaError_t)e));
+        }
+        for (uint32_t m = 0; m < n_mcs; ++m)
+            for (uint32_t k = 0; k < 16; ++k) {
+                if (variant == PGG_VARIANT_LEAN) {
+                    pgg::lean_launch(lplan, fmt, a, m, k, 1, stream, pgg::kGamePGG);
+                } else if (variant == PGG_VARIANT_RING) {
+                    pgg::ring_launch(rplan, fmt, a, m, k, 1, stream);
+                } else {
+                    const uint32_t n_cls = (L / 4) * (L / 4);
+                    dim3 grid((n_cls + 255) / 256, 1);
+                    if (fmt == PGG_FMT_U8)
+                        pgg::phase_v0_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, m, k);
+                    else
+                        pgg::phase_v0_kernel<pgg::kFmtBits><<<grid, 256, 0, stream>>>(a, m, k);
+                }
+                PGG_LAUNCHED();
+            }
+    }
+    if (d_counts != nullptr) {
+        pgg::finalize_counts_kernel<<<1, 1024, 0, stream>>>(reinterpret_cast<unsigned long long*>(d_counts), n_mcs, d_count0);
+        PGG_LAUNCHED();
+    }
+    return PGG_OK;
+}
 
 int32_t pgg_build_accept_table(double r, double K, uint32_t* h_out153)
 {
