@@ -178,7 +178,7 @@ def run_ours(args):
     fmt = pgg.FMT_U8 if args.fmt == "u8" else pgg.FMT_BITS
     variant = {"auto": pgg.VARIANT_AUTO, "v0": pgg.VARIANT_V0, "tile": pgg.VARIANT_TILE,
                "pipe": pgg.VARIANT_PIPE, "band": pgg.VARIANT_BAND,
-               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT, "lean": pgg.VARIANT_LEAN, "persist": pgg.VARIANT_PERSIST, "cluster": pgg.VARIANT_CLUSTER}[args.variant]
+               "ring": pgg.VARIANT_RING, "split": pgg.VARIANT_SPLIT, "dyn": pgg.VARIANT_DYN, "resident": pgg.VARIANT_RESIDENT, "lean": pgg.VARIANT_LEAN, "persist": pgg.VARIANT_PERSIST, "cluster": pgg.VARIANT_CLUSTER, "packed": pgg.VARIANT_PACKED}[args.variant]
     pgg.pgg_set_variant(variant)
     seed = SEED + rank
     shape = (L, L) if fmt == pgg.FMT_U8 else (L, L // 32)
@@ -225,6 +225,9 @@ def run_ours(args):
         step(i)
     barrier()
     launches = pgg.pgg_launch_count() - launches0
+    variant_used = pgg.pgg_get_variant_used()
+    # PACKED: the uint8 lattice is the caller's layout only; the kernels run on a bit-packed working copy
+    packed = variant_used == pgg.VARIANT_PACKED
     clocks = sampler.stop() if rank == 0 else None
     total_ms = ev_a[0].elapsed_time(ev_c[-1])
     sweep_ms = sum(ev_b[i].elapsed_time(ev_c[i]) for i in range(args.steps))
@@ -264,6 +267,33 @@ def run_ours(args):
     e2e_value = job_value(world, e2e_steps, updates_per_step, e2e_ms)
     assert torch.equal(h_counts, last_counts), "e2e run and device-resident run disagree"
 
+    # ---- context for a PACKED run: the same step on the in-place streaming kernel (RING reads the uint8 rows
+    # from HBM every phase), one warm-up + one timed step, so that its HBM fraction stays on record
+    streaming = None
+    if packed and not args.no_streaming_context and pgg.pgg_variant_supported(pgg.VARIANT_RING, fmt, L):
+        pgg.pgg_set_variant(pgg.VARIANT_RING)
+        step()
+        s0, s1, s2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        s0.record(stream)
+        pgg.pgg_init_lattice(d_lat, fmt, L, RHO0, seed, stream)
+        s1.record(stream)
+        pgg.pgg_sweep(d_lat, fmt, L, R, K_NOISE, seed, ORDER, 0, n_mcs, d_counts, stream)
+        s2.record(stream)
+        barrier()
+        assert torch.equal(d_counts.cpu(), last_counts), "RING and PACKED disagree"
+        pgg.pgg_set_variant(variant)
+        us = s1.elapsed_time(s2) * 1e3 / (16 * n_mcs)
+        gbs = (L * L * 17.0 / 16.0) / (us * 1e-6) / 1e9
+        pk, _ = load_peaks()
+        streaming = {"variant": pgg.VARIANT_RING, "kernel": "phase_ring_kernel, in place on the uint8 rows",
+                     "updates_per_s": updates_per_step / (s0.elapsed_time(s2) * 1e-3), "avg_launch_us": us,
+                     "bound": "hbm", "achieved": gbs, "peak": pk, "unit": "GB/s", "frac": gbs / pk,
+                     "algorithmic_bytes_per_launch": L * L * 17.0 / 16.0, "steps": 1}
+        try:
+            streaming["traffic"] = json.loads((ROOT / "profiles" / "traffic.json").read_text()).get(f"u8_L{L}_bytes_per_launch")
+        except (ValueError, OSError):
+            streaming["traffic"] = None
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -299,23 +329,24 @@ def run_ours(args):
     per_mcs = 4 if dtile else 16
     n_phase = per_mcs * n_mcs * args.steps
     phase_us = sweep_ms * 1e3 / n_phase            # includes the per-call order/density/finalize kernels
-    b_site = 1.0 if fmt == pgg.FMT_U8 else 0.125
+    b_site = 1.0 if (fmt == pgg.FMT_U8 and not packed) else 0.125   # of the layout the phase kernel reads
     bytes_per_launch = (L * L + L * L / float(per_mcs)) * b_site   # read the lattice, write the active class
     achieved = bytes_per_launch / (phase_us * 1e-6) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "kernel": ("dtile_part_kernel" if dtile else "phase kernel") + " (variant %d)" % pgg.pgg_get_variant_used(),
+                "kernel": ("dtile_part_kernel" if dtile else
+                           "phase_lean_kernel on the bit-packed working copy" if packed else "phase kernel") + " (variant %d)" % variant_used,
                 "avg_launch_us": phase_us, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "note": ("5 B/update (4 parts x (read N + write N/4)); 16 full Philox draws per domain make this "
                          "schedule ALU-bound, the HBM fraction is context" if dtile else
                          "17 B/update contract bytes (16 phases x (read N + write N/16)), SURVEY 8(d)")
                         + ("; the 32 MiB packed lattice is L2-resident, so this is not a DRAM fraction"
-                           if fmt == pgg.FMT_BITS else "")}
+                           if (fmt == pgg.FMT_BITS or packed) else "")}
     tr = ROOT / "profiles" / "traffic.json"
     if tr.exists():
         try:
             roofline["traffic"] = json.loads(tr.read_text()).get(
-                f"{args.fmt}_L{L}_bytes_per_launch" + ("_dtile" if dtile else ""))
+                f"{'bits' if packed else args.fmt}_L{L}_bytes_per_launch" + ("_dtile" if dtile else ""))
         except (ValueError, OSError):
             pass
     # the ALU view: STEP draws per second against the Philox-only ceiling
@@ -326,10 +357,19 @@ def run_ours(args):
            "note": "achieved = updates/s x the time-averaged fraction of sites that need a draw "
                    "(pgg_count_interface at log-spaced MCS of the same run); peak = pgg_probe_draw_rate, "
                    "a kernel that makes STEP draws only (DESIGN.md section 5)"}
-    if fmt == pgg.FMT_BITS and not dtile:
+    if (fmt == pgg.FMT_BITS or packed) and not dtile:
         # the packed lattice is L2-resident: its bound is the integer pipes, not HBM
         alu.update({"traffic": roofline["traffic"], "kernel": roofline["kernel"], "avg_launch_us": phase_us,
                     "hbm_context": {k: roofline[k] for k in ("achieved", "peak", "frac", "algorithmic_bytes_per_launch")}})
+        if packed:
+            # SURVEY 8(d)'s contract figure for a uint8 lattice, 17 B per update, over the same time: what the
+            # north_star's "% of the HBM roofline" formula gives.  NOT bytes this path moves (see hbm_context).
+            contract = (L * L + L * L / 16.0) / (phase_us * 1e-6) / 1e9
+            alu["hbm_contract_u8"] = {"achieved": contract, "peak": peak, "unit": "GB/s", "frac": contract / peak,
+                                      "note": "updates/s x 17 B / peak (SURVEY 8(d)); the phase kernel reads the 1/8-size "
+                                              "working copy instead of the uint8 rows, so this is not DRAM traffic"}
+            if streaming is not None:
+                alu["streaming_kernel_u8"] = streaming
         roofline = alu
     else:
         roofline["alu_context"] = {k: alu[k] for k in ("achieved", "peak", "unit", "frac", "draw_fraction")}
@@ -337,13 +377,17 @@ def run_ours(args):
     out = {
         "metric": METRIC, "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "u8" if fmt == pgg.FMT_U8 else "u1 (bit-packed u32)",
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": ("u8 (lattice in HBM) / u1 (bit-packed u32 working copy the phases run on)" if packed
+                  else "u8" if fmt == pgg.FMT_U8 else "u1 (bit-packed u32)"),
         "data": "synthetic",
         "config": {"workload": f"C5 throughput: single L={L} lattice, Bernoulli(0.5) init seed 1, r={R}, "
                                f"K={K_NOISE}, {n_mcs} MCS per step (init + sweep + fused rho_C trace)",
                    "fmt": args.fmt, "L": L, "mcs_per_step": n_mcs, "order_mode": args.order,
-                   "variant": pgg.pgg_get_variant_used(),
-                   "l2": ("inputs larger than L2 (256 MiB lattice re-read every phase)" if lat_bytes > 130e6
+                   "variant": variant_used,
+                   "l2": ("the call packs the uint8 lattice into a working copy of 1/8 its size, which fits L2; "
+                          "no flush between phases (there is none in the workload)" if packed and lat_bytes / 8 < 120e6
+                          else "inputs larger than L2 (256 MiB lattice re-read every phase)" if lat_bytes > 130e6
                           else "lattice fits L2 by nature of the workload; no flush"),
                    "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
         "mcs_per_s": world * args.steps * n_mcs / (total_ms * 1e-3),
@@ -394,12 +438,14 @@ def main():
     ap.add_argument("--fmt", default="u8", choices=["u8", "bits"])
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--mcs", type=int, default=1000)
-    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "pipe", "band", "ring", "split", "dyn", "resident", "lean", "persist", "cluster"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "v0", "tile", "pipe", "band", "ring", "split", "dyn", "resident", "lean", "persist", "cluster", "packed"])
     ap.add_argument("--order", default="iid", choices=["iid", "perm", "dtile"],
                     help="schedule: the 16-sublattice schedule with i.i.d. (bench default) or permuted classes, or "
                          "the paper's own double-tiling schedule (PAPER.md:75-93); anything but iid is not the bench workload")
     ap.add_argument("--r", type=float, default=R, help="synergy factor; anything but 3.8 is not the bench workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-streaming-context", action="store_true",
+                    help="skip the extra RING step a PACKED run adds for context (roofline.streaming_kernel_u8)")
     ap.add_argument("--profile-mcs", type=int, default=-1,
                     help="profiling aid: bracket this MCS with cudaProfilerStart/Stop (ncu --profile-from-start off); "
                          "the run's numbers are then not bench values")

@@ -104,9 +104,16 @@ enum {
                                 bits on arrival (uint8), scan / draw / stencil on a bit ring   */
     PGG_VARIANT_PERSIST = 12,/* LEAN, bit-packed, <= 148 lattices: every phase of up to 4096 MCS in ONE
                                 cooperative launch, a per-lattice barrier between phases           */
-    PGG_VARIANT_CLUSTER = 13 /* L = 128 .. 4096 (a power of two), both layouts: the lattice stays bit-packed in
+    PGG_VARIANT_CLUSTER = 13,/* L = 128 .. 4096 (a power of two), both layouts: the lattice stays bit-packed in
                                 the shared memory of a CTA cluster (1 .. 16 CTAs) for the whole call, halo rows
                                 over distributed shared memory, one cluster barrier per phase          */
+    PGG_VARIANT_PACKED = 14  /* uint8 lattices, L = 1024 .. 32768 (a power of two): the call packs the lattice
+                                into a bit-packed WORKING COPY (L*L/8 bytes per lattice from the stream-ordered
+                                pool: 32 MiB at L = 16384, which stays in the 126 MB L2), runs every phase on
+                                it with LEAN, and unpacks it into the caller's uint8 lattice when the call ends
+                                (the internal layout SURVEY 8(b) allows behind the canonical ones).  The
+                                caller's lattice holds the result when the call's work on the stream is done,
+                                as always; while the call runs it holds the state the call started from.  */
 };
 
 /* Acceptance table, Eq. (3) PAPER.md:60 in the integer form of SURVEY 8(c) D3:
@@ -239,6 +246,12 @@ int32_t pgg_probe_draw_rate(uint32_t iters, uint64_t seed, uint64_t* h_n_draws, 
 int32_t pgg_count_interface(const void* d_lat, int32_t fmt, uint32_t L, uint64_t* d_count, void* stream);
 
 /* Number of kernels this library has launched in this process (monotone).       */
+/* Temporaries (seeds, tables, class order, the PGG_VARIANT_PACKED working copy) come from a stream-ordered
+ * memory pool the library owns, one per device; what a call frees stays in that pool for the next call
+ * (at most the largest working set calls have had in flight at once).  This returns the unused part to the
+ * driver for the current device; memory of calls still running on a stream is kept.  Errors: PGG_ERR_CUDA. */
+int32_t pgg_trim_workspace(void);
+
 uint64_t pgg_launch_count(void);
 
 /* Text of the last error on the calling thread ("" if none).                    */

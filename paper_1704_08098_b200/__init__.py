@@ -23,7 +23,7 @@ FMT_U8, FMT_BITS = 0, 1
 ORDER_IID, ORDER_PERM, ORDER_DTILE = 0, 1, 2
 VARIANT_AUTO, VARIANT_V0, VARIANT_TILE = 0, 1, 2
 VARIANT_PIPE, VARIANT_BAND, VARIANT_RING, VARIANT_SPLIT, VARIANT_DYN, VARIANT_RESIDENT = 4, 5, 6, 7, 8, 9
-VARIANT_DTILE, VARIANT_LEAN, VARIANT_PERSIST, VARIANT_CLUSTER = 10, 11, 12, 13
+VARIANT_DTILE, VARIANT_LEAN, VARIANT_PERSIST, VARIANT_CLUSTER, VARIANT_PACKED = 10, 11, 12, 13, 14
 
 # name -> (restype, argtypes); also the list of symbols include/pgg.h declares
 _u32p, _u64p, _u8p, _f64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_uint8),
@@ -49,6 +49,7 @@ SIGNATURES = {
     "pgg_variant_supported": (C.c_int32, [C.c_int32, C.c_int32, C.c_uint32]),
     "pgg_probe_draw_rate": (C.c_int32, [C.c_uint32, C.c_uint64, _u64p, C.c_void_p]),
     "pgg_count_interface": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_void_p, C.c_void_p]),
+    "pgg_trim_workspace": (C.c_int32, []),
     "pgg_launch_count": (C.c_uint64, []),
     "pgg_last_error": (C.c_char_p, []),
 }
@@ -174,6 +175,11 @@ def pgg_probe_draw_rate(iters: int, seed: int = 1, stream=None) -> int:
 
 def pgg_count_interface(d_lat, fmt: int, L: int, d_count, stream=None) -> None:
     _check(lib().pgg_count_interface(_ptr(d_lat), fmt, L, _ptr(d_count), _stream(stream)))
+
+
+def pgg_trim_workspace() -> None:
+    """Give the unused part of the library's memory pool (current device) back to the driver."""
+    _check(lib().pgg_trim_workspace())
 
 
 def pgg_launch_count() -> int:

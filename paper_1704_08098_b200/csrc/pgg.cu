@@ -79,6 +79,39 @@ inline unsigned long long lattice_bytes(int32_t fmt, uint32_t L)
     return fmt == PGG_FMT_U8 ? n : n / 8;
 }
 
+// The library's own stream-ordered memory pool, one per device, created on first use.  Its release
+// threshold is unlimited: what a call frees stays in the pool for the next call instead of going back
+// to the driver at the next synchronisation (the default pool does that, and a call that needs a 32 MiB
+// working copy would then pay a fresh allocation every time).  pgg_trim_workspace() gives it back.
+constexpr int kMaxDevices = 64;
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pool[kMaxDevices] = {};
+
+cudaError_t workspace_pool(cudaMemPool_t* out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pool[dev] == nullptr) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        e = cudaMemPoolCreate(&pool, &props);
+        if (e != cudaSuccess) return e;
+        unsigned long long keep = ~0ull;
+        e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) return e;
+        g_pool[dev] = pool;
+    }
+    *out = g_pool[dev];
+    return cudaSuccess;
+}
+
 // Device temporaries of one call, returned to the stream-ordered pool on scope exit.
 struct Scratch {
     cudaStream_t stream;
@@ -90,7 +123,10 @@ struct Scratch {
     }
     cudaError_t alloc(void** p, size_t bytes)
     {
-        cudaError_t e = cudaMallocAsync(p, bytes ? bytes : 16, stream);
+        cudaMemPool_t pool = nullptr;
+        cudaError_t e = workspace_pool(&pool);
+        if (e != cudaSuccess) return e;
+        e = cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, stream);
         if (e == cudaSuccess) ptrs.push_back(*p);
         return e;
     }
@@ -195,9 +231,15 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         // L = 1024: 2.8 against 4.3 for one lattice, 8.7 against 11.9 for 64; L = 2048 from 32 lattices
         // (28.7 against 33 / 52 at 64); never at L = 4096 (16 CTAs per lattice leave the GPU idle)
         const bool cluster_pays = pgg::cluster_supported(fmt, L) && (L == 512 || L == 1024 || (L == 2048 && B >= 32));
+        // uint8 at L >= 2048 (powers of two): a bit-packed working copy for the length of the call and LEAN on it
+        // (PACKED).  The copy is 1/8 of the lattice -- 32 MiB at L = 16384, L2-resident -- and LEAN's phase on
+        // it takes 45 us against RING's 60 on the uint8 rows; packing and unpacking cost two passes per CALL.
+        static const uint32_t packed_min_L = [] { const char* e = getenv("PGG_PACKED_MIN_L"); return e ? (uint32_t)atoi(e) : 2048u; }();
+        const bool packed_pays = fmt == PGG_FMT_U8 && !pd && pgg::lean_supported(PGG_FMT_BITS, L) && L >= packed_min_L;
         variant = cluster_pays ? PGG_VARIANT_CLUSTER
                 : (res_ok && res_pays) ? PGG_VARIANT_RESIDENT
                 : lean_bits ? PGG_VARIANT_LEAN
+                : packed_pays ? PGG_VARIANT_PACKED
                 : !stream_pays ? PGG_VARIANT_V0
                 : (fmt == PGG_FMT_U8 && ring_ok) ? PGG_VARIANT_RING : band_ok ? PGG_VARIANT_BAND : PGG_VARIANT_V0;
     }
@@ -217,6 +259,8 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_LEAN && !pgg::lean_supported(fmt, L))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
+    if (variant == PGG_VARIANT_PACKED && !(fmt == PGG_FMT_U8 && !pd && pgg::lean_supported(PGG_FMT_BITS, L)))
+        return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_CLUSTER && !pgg::cluster_supported(fmt, L))
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     if (variant == PGG_VARIANT_PERSIST && !pgg::lean_persist_supported(fmt, L, B))
@@ -228,6 +272,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     if ((variant == PGG_VARIANT_TILE || variant == PGG_VARIANT_PIPE) && !tile_ok)
         return fail(PGG_ERR_UNSUPPORTED, "variant %d does not support fmt %d, L %u", variant, fmt, L);
     g_variant_used = variant;
+    // PACKED: the kernels see a bit-packed working copy and run LEAN; the caller's layout stays uint8
+    const bool packed = variant == PGG_VARIANT_PACKED;
+    const int kfmt = packed ? PGG_FMT_BITS : fmt;
+    if (packed) variant = PGG_VARIANT_LEAN;
 
     Scratch tmp(stream);
     // per-lattice seeds and acceptance tables
@@ -286,10 +334,17 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
     }
     uint8_t* d_order = nullptr;
     PGG_CUDA(tmp.alloc((void**)&d_order, (size_t)B * chunk * 16));
+    uint8_t* d_work = d_lats;
+    const unsigned long long n_words = (unsigned long long)B * L * L / 32ull;
+    if (packed) {
+        PGG_CUDA(tmp.alloc((void**)&d_work, (size_t)(4ull * n_words)));
+        pgg::packed_launch(true, d_lats, d_work, n_words, stream);
+        PGG_LAUNCHED();
+    }
 
     pgg::PhaseArgs a;
-    a.lats = d_lats;
-    a.lat_bytes = lattice_bytes(fmt, L);
+    a.lats = d_work;
+    a.lat_bytes = lattice_bytes(kfmt, L);
     a.seeds = d_seeds;
     a.tables = d_tables;
     a.order = d_order;
@@ -338,7 +393,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         PGG_CUDA(tmp.alloc((void**)&d_gbar, sizeof(unsigned int) * B));
     }
     if (variant == PGG_VARIANT_LEAN || variant == PGG_VARIANT_PERSIST) {
-        int32_t rc = pgg::lean_plan(fmt, L, B, &lplan);
+        int32_t rc = pgg::lean_plan(kfmt, L, B, &lplan);
         if (rc != 0) return fail(PGG_ERR_CUDA, "lean kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
     }
     pgg::ResPlan resplan;
@@ -370,7 +425,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         for (uint32_t m = m0; m < m0 + n_chunk; ++m) {
             for (uint32_t k = 0; k < 16; ++k) {
                 if (variant == PGG_VARIANT_LEAN) {
-                    pgg::lean_launch(lplan, fmt, a, m, k, B, stream, game);
+                    pgg::lean_launch(lplan, kfmt, a, m, k, B, stream, game);
                 } else if (variant == PGG_VARIANT_DYN) {
                     pgg::dyn_launch(rplan, a, m, k, B, stream);
                 } else if (variant == PGG_VARIANT_SPLIT) {
@@ -398,6 +453,10 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
                 PGG_LAUNCHED();
             }
         }
+    }
+    if (packed) {  // the working copy -> the caller's uint8 lattice
+        pgg::packed_launch(false, d_lats, d_work, n_words, stream);
+        PGG_LAUNCHED();
     }
     if (d_counts != nullptr) {
         pgg::finalize_counts_kernel<<<B, 1024, 0, stream>>>(
@@ -681,7 +740,7 @@ int32_t pgg_phase_classes(uint64_t seed, uint32_t t, int32_t order_mode, uint8_t
 
 int32_t pgg_set_variant(int32_t variant)
 {
-    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_CLUSTER || variant == PGG_VARIANT_DTILE || variant == 3)
+    if (variant < PGG_VARIANT_AUTO || variant > PGG_VARIANT_PACKED || variant == PGG_VARIANT_DTILE || variant == 3)
         return fail(PGG_ERR_UNSUPPORTED, "unknown variant %d", variant);
     g_variant.store(variant);
     return PGG_OK;
@@ -703,6 +762,7 @@ int32_t pgg_variant_supported(int32_t variant, int32_t fmt, uint32_t L)
     if (variant == PGG_VARIANT_LEAN) return pgg::lean_supported(fmt, L) ? 1 : 0;
     if (variant == PGG_VARIANT_PERSIST) return pgg::lean_persist_supported(fmt, L, 1) ? 1 : 0;
     if (variant == PGG_VARIANT_CLUSTER) return pgg::cluster_supported(fmt, L) ? 1 : 0;
+    if (variant == PGG_VARIANT_PACKED) return (fmt == PGG_FMT_U8 && pgg::lean_supported(PGG_FMT_BITS, L)) ? 1 : 0;
     return 0;
 }
 
@@ -741,6 +801,16 @@ int32_t pgg_count_interface(const void* d_lat, int32_t fmt, uint32_t L, uint64_t
         pgg::interface_count_kernel<pgg::kFmtBits><<<grid, 256, 0, s>>>(static_cast<const uint8_t*>(d_lat), L,
                                                                       reinterpret_cast<unsigned long long*>(d_count));
     PGG_LAUNCHED();
+    return PGG_OK;
+}
+
+int32_t pgg_trim_workspace(void)
+{
+    int dev = -1;
+    PGG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(PGG_ERR_UNSUPPORTED, "device ordinal %d", dev);
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pool[dev] != nullptr) PGG_CUDA(cudaMemPoolTrimTo(g_pool[dev], 0));
     return PGG_OK;
 }
 

@@ -34,7 +34,7 @@ namespace cg = cooperative_groups;
 
 constexpr int kClusterWarps = 16;
 constexpr int kClusterThreads = kClusterWarps * 32;
-constexpr int kClusterFixedBytes = kClusterWarps * kLeanWarpQBytes + 160 * 4 + 8 * 4 + 128;
+constexpr int kClusterFixedBytes = kClusterWarps * kLeanWarpQBytes + 160 * 4 + 8 * 4 + kStencilLutBytes + 128;
 
 struct ClusterPlan {
     uint32_t lg2L;
@@ -62,6 +62,7 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
     const int q_off = (int)(rows + 6) * pitch;
     uint32_t* tbl = reinterpret_cast<uint32_t*>(smem_raw + q_off + kClusterWarps * kLeanWarpQBytes);
     int* eoff = reinterpret_cast<int*>(tbl + 160);
+    int8_t* lut = reinterpret_cast<int8_t*>(eoff + 8);  // StencilLut (pgg_kernels_lean.cuh)
     __shared__ int delta_cta;
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
 
@@ -81,6 +82,9 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
         words[idx] = w;
     }
     for (int q = threadIdx.x; q < kTableSize; q += kClusterThreads) tbl[q] = a.tables[(size_t)b * kTableSize + q];
+    if (GAME == kGamePGG)
+        for (int q = threadIdx.x; q < kStencilLutBytes / 4; q += kClusterThreads)
+            reinterpret_cast<uint32_t*>(lut)[q] = reinterpret_cast<const uint32_t*>(g_stencil_lut.v)[q];
     if (threadIdx.x == 0) {
         delta_cta = 0;
         const int ps = (int)L;  // one row down, in bits
@@ -131,7 +135,7 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
             } else {
                 const int dA = (col < 3 || col > colmask - 3)
                                    ? ring_stencil_fr<kFmtBits>(soff, dir, sx, ring0, 0, colmask)
-                                   : ring_stencil<kFmtBits, false>(soff, dir, sx, ring0, eoff, 0);
+                                   : bits_stencil_lut(soff, dir, sx, reinterpret_cast<const uint32_t*>(ring0), wpr, lut);
                 idx_t = sx * 102 + dA + 25;
             }
             if (w.z < tbl[idx_t]) {

@@ -61,7 +61,8 @@ constexpr int kLeanWarpQBytes = kLeanQ1Cap * 8 + kLeanQ2Cap * 16;
 constexpr int kLeanMaxSlots = 12; // staging slots (uint8) / ring chunks (bit-packed): barrier array size
 constexpr int kLeanLagU8 = 4;     // ring chunks >= lag + 3 (see "Queue lifetime"); the rest runs ahead
 constexpr int kLeanLagBits = 8;
-constexpr int kLeanFixedBytes = kLeanConsumers * kLeanWarpQBytes + 160 * 4 + 4 * kLeanMaxSlots * 8 + 8 * 4 + 128;
+constexpr int kStencilLutBytes = 4 * 6 * 128;  // StencilLut below
+constexpr int kLeanFixedBytes = kLeanConsumers * kLeanWarpQBytes + 160 * 4 + 4 * kLeanMaxSlots * 8 + 8 * 4 + kStencilLutBytes + 128;
 
 struct LeanPlan {
     uint32_t lg2L;       // L = 2^lg2L sites per row = bits per ring row
@@ -116,6 +117,61 @@ __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
+// ---------------------------------------------------------------------------
+// The payoff stencil on bit rows by table (a5).  A_x - A_y is a signed sum over 12 neighbours of x
+// (ring_stencil: offsets a e + b f, e = step towards y, f = the perpendicular step) plus 3 (2 s_x - 1).
+// The 12 sites lie in six rows -- a = -2 .. 3 for a vertical e, b = -2 .. 2 (and a spare) for a horizontal
+// e -- and, in every row, in the seven columns col(x) - 3 .. col(x) + 3.  So per row: the 7-bit window
+// (two word loads, a funnel shift, a mask) indexes a 128-entry table that holds the row's weighted sum:
+// six table reads replace fourteen single-bit reads (5 instructions each).  Sites within 3 columns of a
+// row end keep the wrapping path (ring_stencil_fr).
+//   lut[dir][slot][window] : int8, 4 x 6 x 128 = 3072 bytes, copied to shared memory by every CTA
+//   slot s of dir: ring row of x + (s - 2) * step(dir),  step = -1 row for dir 0 (e points up), else +1 row
+// ---------------------------------------------------------------------------
+struct StencilLut {
+    int8_t v[4 * 6 * 128];
+};
+static_assert(sizeof(StencilLut) == kStencilLutBytes, "StencilLut size");
+
+constexpr StencilLut make_stencil_lut()
+{
+    StencilLut t{};
+    // (a, b, weight): x's 13-site weights minus y's, y = x + e, without the centre pair (include/pgg.h)
+    const int term[12][3] = {{-2, 0, 1}, {-1, 0, 1}, {2, 0, -1}, {3, 0, -1}, {-1, 1, 2}, {-1, -1, 2},
+                             {2, 1, -2}, {2, -1, -2}, {0, 2, 1}, {0, -2, 1}, {1, 2, -1}, {1, -2, -1}};
+    for (int dir = 0; dir < 4; ++dir) {
+        // e = (er, ec), f = (fr, fc) in (rows, columns): the directions of SURVEY 8(c) D6 and eoff[4..7]
+        const int er = dir == 0 ? -1 : dir == 1 ? 1 : 0, ec = dir == 2 ? -1 : dir == 3 ? 1 : 0;
+        const int fr = dir < 2 ? 0 : 1, fc = dir < 2 ? 1 : 0;
+        const int step = dir == 0 ? -1 : 1;  // rows per slot
+        for (int q = 0; q < 12; ++q) {
+            const int dr = term[q][0] * er + term[q][1] * fr, dc = term[q][0] * ec + term[q][1] * fc;
+            const int slot = dr * step + 2;  // dr = (slot - 2) * step
+            for (int w = 0; w < 128; ++w)
+                if ((w >> (dc + 3)) & 1) t.v[(dir * 6 + slot) * 128 + w] += (int8_t)term[q][2];
+        }
+    }
+    return t;
+}
+__device__ const StencilLut g_stencil_lut = make_stencil_lut();
+
+// lut = the table in shared memory; words = ring0 as 32-bit words; wpr = words per ring row.
+// Needs 3 <= col(x) <= L - 4 (the window stays inside the row); the word after the window's first is
+// read even when the window does not reach it (the ring is followed by the queues: a valid address).
+__device__ __forceinline__ int bits_stencil_lut(int soff, uint32_t dir, int sx, const uint32_t* words, int wpr, const int8_t* lut)
+{
+    const int base = soff - 3;
+    const uint32_t sh = (uint32_t)base & 31u;
+    const int stepw = dir == 0u ? -wpr : wpr;
+    const uint32_t* p = words + (base >> 5) - 2 * stepw;
+    const int8_t* l = lut + dir * 768u;
+    int dA = 3 * (2 * sx - 1);
+#pragma unroll
+    for (int s = 0; s < 6; ++s, p += stepw)
+        dA += l[s * 128 + (__funnelshift_r(p[0], p[1], sh) & 127u)];
+    return dA;
+}
+
 // SRC = layout of the lattice in global memory (kFmtU8 / kFmtBits); the ring is always bits.
 // Warps 0..15: workers.  Warp 16: producer (bulk copies).  Warps 17..20 (uint8 only): packers.
 // GAME = kGamePGG (the 14-read payoff stencil) or kGamePD (neighbour counts of x and y).
@@ -137,6 +193,7 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
     uint32_t* tbl = reinterpret_cast<uint32_t*>(smem_raw + q_off + kLeanConsumers * kLeanWarpQBytes);
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(tbl + 160);  // ring full[], ring empty[], stage full[], stage empty[]
     int* eoff = reinterpret_cast<int*>(bars + 4 * kLeanMaxSlots);                 // e[4], f[4]
+    int8_t* lut = reinterpret_cast<int8_t*>(eoff + 8);                            // StencilLut
     __shared__ int delta_cta;
 
     const uint32_t b = blockIdx.y;
@@ -149,6 +206,9 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
     if (!PERSIST) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (int q = threadIdx.x; q < kTableSize; q += blockDim.x)
         tbl[q] = a.tables[(size_t)b * kTableSize + q];
+    if (GAME == kGamePGG)
+        for (int q = threadIdx.x; q < kStencilLutBytes / 4; q += blockDim.x)
+            reinterpret_cast<uint32_t*>(lut)[q] = reinterpret_cast<const uint32_t*>(g_stencil_lut.v)[q];
     if (threadIdx.x == 0) {
         delta_cta = 0;
         for (uint32_t s = 0; s < NR; ++s) {
@@ -322,7 +382,7 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
             } else {
                 const int dA = (col < 3 || col > colmask - 3)
                                    ? ring_stencil_fr<kFmtBits>(soff, dir, sx, ring0, 0, colmask)
-                                   : ring_stencil<kFmtBits, false>(soff, dir, sx, ring0, eoff, 0);
+                                   : bits_stencil_lut(soff, dir, sx, reinterpret_cast<const uint32_t*>(ring0), pitch >> 2, lut);
                 idx_t = sx * 102 + dA + 25;  // table_index(dA, ds) with ds = 2 s_x - 1
             }
             if (w.z < tbl[idx_t]) {
@@ -511,6 +571,47 @@ sweep_lean_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, LeanPlan g, unsigned
         }
         __syncthreads();
     }
+}
+
+// ---------------------------------------------------------------------------
+// PGG_VARIANT_PACKED: uint8 lattices <-> a bit-packed working copy (pure layout: bit j & 31 of word
+// i (L/32) + (j >> 5) = byte (i, j), include/pgg.h).  One 32-site word per thread and trip: two 16-byte
+// loads -> one 4-byte store, and back.  n_words = B L^2 / 32 over all lattices (they are contiguous in both).
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+pack_u8_kernel(const uint8_t* __restrict__ src, uint32_t* __restrict__ dst, unsigned long long n_words)
+{
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += stride) {
+        const uint4* p = reinterpret_cast<const uint4*>(src) + 2ull * w;
+        const uint4 v0 = __ldcs(p), v1 = __ldcs(p + 1);  // read once: do not displace the working copy from L2
+        dst[w] = (lean_pack16(v0) & 0xFFFFu) | (lean_pack16(v1) << 16);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+unpack_u8_kernel(const uint32_t* __restrict__ src, uint8_t* __restrict__ dst, unsigned long long n_words)
+{
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += stride) {
+        const uint32_t v = src[w];
+        uint32_t o[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {  // four sites per 32-bit word, one byte each
+            const uint32_t nib = (v >> (4 * q)) & 0xFu;
+            o[q] = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);
+        }
+        uint4* p = reinterpret_cast<uint4*>(dst) + 2ull * w;
+        __stcs(p, make_uint4(o[0], o[1], o[2], o[3]));
+        __stcs(p + 1, make_uint4(o[4], o[5], o[6], o[7]));
+    }
+}
+
+inline void packed_launch(bool pack, uint8_t* d_u8, uint8_t* d_bits, unsigned long long n_words, cudaStream_t stream)
+{
+    const uint32_t grid = (uint32_t)std::min<unsigned long long>((n_words + 255ull) / 256ull, 148ull * 16ull);
+    if (pack) pack_u8_kernel<<<grid, 256, 0, stream>>>(d_u8, reinterpret_cast<uint32_t*>(d_bits), n_words);
+    else unpack_u8_kernel<<<grid, 256, 0, stream>>>(reinterpret_cast<const uint32_t*>(d_bits), d_u8, n_words);
 }
 
 // ---------------------------------------------------------------------------

@@ -26,21 +26,38 @@ def test_bench_line_has_the_contract_keys():
                 "vs_baseline", "dtype", "data", "config", "e2e", "gpu_launches", "clocks", "roofline", "cpu_baseline"):
         assert key in d, key
     assert d["unit"] == "updates/s" and d["n_gpus"] == 1 and d["steps"] == 2 and d["warmup"] == 3
-    assert d["dtype"] == "u8" and d["data"] == "synthetic" and d["vs_baseline"] is None
+    assert d["dtype"].startswith("u8") and d["data"] == "synthetic" and d["vs_baseline"] is None
     assert "workload" in d["config"] and "model" not in d["config"]
+    assert d["config"]["variant"] == 14                   # AUTO -> PACKED for a uint8 lattice of L = 2048
     assert d["value"] > 0 and d["e2e"]["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] == 2048 * 2048 and d["e2e"]["d2h_bytes_per_step"] > 2048 * 2048
-    # (seed upload + init) + (seed/table upload + density + order + 16 phases per MCS + finalize), per step
-    assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 1 + 16 * 20 + 1))
-    r = d["roofline"]
-    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
-    a = r["alu_context"]                                  # the draws against the Philox-only ceiling
-    assert a["unit"] == "Gdraw/s" and 0.0 < a["draw_fraction"] <= 1.0 and 0.0 < a["frac"] < 1.5
+    # (seed upload + init) + (seed/table upload + density + pack + order + 16 phases per MCS + unpack + finalize), per step
+    assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 1 + 1 + 16 * 20 + 1 + 1))
+    r = d["roofline"]                                     # the phases run on the packed working copy: ALU-bound
+    assert r["bound"] == "alu" and r["unit"] == "Gdraw/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert 0.0 < r["draw_fraction"] <= 1.0 and r["hbm_context"]["algorithmic_bytes_per_launch"] == 2048 * 2048 * 17 / 16 / 8
+    c8 = r["hbm_contract_u8"]                             # the north_star's formula: updates/s x 17 B / peak
+    assert abs(c8["achieved"] - 8.0 * r["hbm_context"]["achieved"]) < 1e-6 * c8["achieved"]
+    st = r["streaming_kernel_u8"]                         # the in-place streaming kernel, timed in the same run
+    assert st["variant"] == 6 and st["bound"] == "hbm" and st["algorithmic_bytes_per_launch"] == 2048 * 2048 * 17 / 16
+    assert st["updates_per_s"] > 0 and abs(st["frac"] - st["achieved"] / st["peak"]) < 1e-9
     assert d["ceilings"]["philox_step_draws_per_s"] > 1e10
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == "updates/s"
     assert c["one_thread"]["cores"] == 1 and c["one_thread"]["value"] > 0 and "MCS 0" in c["sample"]
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+def test_bench_line_for_the_streaming_kernel():
+    """--variant ring: in place on the uint8 rows, the HBM roofline with the 17 B/update contract bytes."""
+    d = run_bench("--variant", "ring", "--no-cpu-baseline")
+    assert d["dtype"] == "u8" and d["config"]["variant"] == 6
+    assert d["gpu_launches"] == 2 * ((1 + 1) + (1 + 1 + 1 + 16 * 20 + 1))
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert r["algorithmic_bytes_per_launch"] == 2048 * 2048 * 17 / 16
+    a = r["alu_context"]                                  # SURVEY 8(d)(ii): the draws against the Philox-only ceiling
+    assert a["unit"] == "Gdraw/s" and 0.0 < a["draw_fraction"] <= 1.0 and 0.0 < a["frac"] < 1.5
 
 
 def test_bench_reference_arm_line():

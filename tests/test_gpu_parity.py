@@ -17,7 +17,7 @@ import paper_1704_08098_b200 as pgg  # noqa: E402
 K = wl.K_DEFAULT
 FMTS = [pgg.FMT_U8, pgg.FMT_BITS]
 VARIANTS = [pgg.VARIANT_V0, pgg.VARIANT_TILE, pgg.VARIANT_PIPE, pgg.VARIANT_BAND, pgg.VARIANT_RING, pgg.VARIANT_SPLIT, pgg.VARIANT_DYN,
-            pgg.VARIANT_RESIDENT, pgg.VARIANT_LEAN]
+            pgg.VARIANT_RESIDENT, pgg.VARIANT_LEAN, pgg.VARIANT_PACKED]
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -371,7 +371,7 @@ def test_oversubscribed_ensemble(fmt):
 def test_fullrow_strip_sizes(L):
     """uint8 lattices whose row is one strip (512 B ... 8 KB): staged without halo columns, one bulk copy
     per chunk, column wrap resolved in the sites near a row end (RING full-row mode)."""
-    pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+    pgg.pgg_set_variant(pgg.VARIANT_RING)
     seed, r, n_mcs = 40 + L, 3.8, 2
     lat0 = orc.init(L, 0.5, seed)
     ref = lat0.copy()
@@ -412,6 +412,7 @@ LONG_CASES = [
     ("PERSIST", pgg.FMT_BITS, 1024, {}),                         # LEAN, one cooperative launch per 4096 MCS
     ("CLUSTER", pgg.FMT_U8, 1024, {}),                           # lattice resident in a cluster's shared memory
     ("CLUSTER", pgg.FMT_BITS, 1024, {}),
+    ("PACKED", pgg.FMT_U8, 1024, {}),                            # uint8 in HBM, bit-packed working copy + LEAN (C5's path)
 ]
 
 
@@ -440,7 +441,7 @@ def test_one_call_longer_than_an_order_chunk(name, fmt, L, env, monkeypatch):
 
 
 @pytest.mark.parametrize("name,fmt,L,env", LONG_CASES,
-                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits", "PERSIST-bits", "CLUSTER-u8", "CLUSTER-bits"])
+                         ids=["RING-fullrow", "RING-strips", "BAND-bits", "LEAN-u8", "LEAN-bits", "PERSIST-bits", "CLUSTER-u8", "CLUSTER-bits", "PACKED-u8"])
 @pytest.mark.parametrize("t0", [99900, 2**32 - 40])
 def test_streaming_kernels_late_windows(name, fmt, L, env, t0, monkeypatch):
     """SURVEY 8(d) late windows (t = 99 900) and the counter width (t_begin + m up to 2^32 - 1)

@@ -124,6 +124,10 @@ def test_variant_support_table():
     # SPLIT and DYN are uint8 only
     assert sup(pgg.VARIANT_SPLIT, pgg.FMT_U8, 2048) and not sup(pgg.VARIANT_SPLIT, pgg.FMT_BITS, 2048)
     assert sup(pgg.VARIANT_DYN, pgg.FMT_U8, 2048) and not sup(pgg.VARIANT_DYN, pgg.FMT_BITS, 2048)
+    # PACKED is uint8 in HBM with a bit-packed working copy for LEAN: LEAN's sizes, uint8 only
+    assert sup(pgg.VARIANT_PACKED, pgg.FMT_U8, 1024) and sup(pgg.VARIANT_PACKED, pgg.FMT_U8, 32768)
+    assert not sup(pgg.VARIANT_PACKED, pgg.FMT_BITS, 1024) and not sup(pgg.VARIANT_PACKED, pgg.FMT_U8, 512)
+    assert not sup(pgg.VARIANT_PACKED, pgg.FMT_U8, 3072)
     assert not sup(99, pgg.FMT_U8, 64)
 
 

@@ -58,7 +58,7 @@ def run_pair(sweep, fmt, L, n1, n2, with_counts=True):
     return out, used_a
 
 
-# (fmt, L, kernel the AUTO rule picks for one lattice, MCS of the two calls)
+# (fmt, L, kernel pgg_sweep_static picks, MCS of the two calls)
 CASES = [
     (pgg.FMT_U8, 128, pgg.VARIANT_RESIDENT, 12, 9),
     (pgg.FMT_BITS, 128, pgg.VARIANT_RESIDENT, 12, 9),
@@ -73,9 +73,9 @@ CASES = [
 
 @pytest.mark.parametrize("fmt,L,kernel,n1,n2", CASES)
 def test_static_sweep_equals_sweep_on_two_calls_in_a_row(fmt, L, kernel, n1, n2):
-    ref, used_ref = run_pair(pgg.pgg_sweep, fmt, L, n1, n2)
+    ref, _ = run_pair(pgg.pgg_sweep, fmt, L, n1, n2)  # (its AUTO choice may differ: PACKED needs a working copy)
     got, used = run_pair(pgg.pgg_sweep_static, fmt, L, n1, n2)
-    assert used == kernel and used_ref == kernel, (used, used_ref, kernel)
+    assert used == kernel, (used, kernel)
     for what, x, y in zip(("lattice A", "lattice B", "counts A", "counts B"), got, ref):
         assert np.array_equal(x, y), f"{what}: {int((x != y).sum())} mismatches"
     assert got[2].min() >= 0 and got[3].min() >= 0  # every count written
