@@ -79,8 +79,9 @@ enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
 
 /* Kernel variants of the phase step (all bit-identical).
  * PGG_VARIANT_AUTO picks by measurement (DESIGN.md appendix B): CLUSTER for L = 512 and 1024 and for
- * L = 2048 from 32 lattices; else RESIDENT for L <= 320 and for L <= 448 from 3 lattices; else LEAN for the
- * bit-packed layout at L = 1024 .. 32768 (powers of two); else RING (uint8) / BAND (bit-packed) for
+ * L = 2048 from 32 lattices; else RESIDENT for L <= 320 and for L <= 448 from 3 lattices; else, for
+ * L = 1024 .. 32768 (powers of two), LEAN for the bit-packed layout and PACKED (a bit-packed working copy +
+ * LEAN) for uint8 from L = 2048; else RING (uint8) / BAND (bit-packed) for
  * L >= 2048 and for uint8 L = 512; else V0.  TILE, PIPE, SPLIT, DYN, BAND (uint8), PERSIST are rungs of the
  * ladder kept for comparison: selectable, tested, never chosen.  Tuning knobs read from the environment by
  * the plan functions (defaults are the measured best; every setting is bit-exact): PGG_PDL,

@@ -13,12 +13,12 @@ from __future__ import annotations
 
 import sys
 
-from . import (FMT_BITS, FMT_U8, ORDER_IID, VARIANT_AUTO, VARIANT_BAND, VARIANT_CLUSTER, VARIANT_LEAN, VARIANT_RESIDENT, VARIANT_RING,
+from . import (FMT_BITS, FMT_U8, ORDER_IID, VARIANT_AUTO, VARIANT_BAND, VARIANT_CLUSTER, VARIANT_LEAN, VARIANT_PACKED, VARIANT_RESIDENT, VARIANT_RING,
                VARIANT_V0, pgg_density, pgg_run_ensemble, pgg_set_variant, pgg_variant_supported)
 
 K = 0.5
 NAMES = {VARIANT_V0: "V0", VARIANT_RESIDENT: "RESIDENT", VARIANT_RING: "RING", VARIANT_BAND: "BAND", VARIANT_LEAN: "LEAN",
-         VARIANT_CLUSTER: "CLUSTER"}
+         VARIANT_CLUSTER: "CLUSTER", VARIANT_PACKED: "PACKED"}
 
 
 def time_variant(variant, fmt, B, L, r, warm, n):
@@ -70,13 +70,13 @@ def main():
         shapes = [(16, 2048, 3.7446, 2000, 200), (16, 2048, 3.8, 500, 200), (1, 4096, 3.7446, 1000, 200),
                   (16, 4096, 3.7446, 1000, 100), (1, 8192, 3.8, 300, 100), (64, 1024, 3.75, 500, 200)]
         cases = [(fmt, B, L, r, warm, n) for (B, L, r, warm, n) in shapes for fmt in (FMT_U8, FMT_BITS)]
-        variants = [VARIANT_RING, VARIANT_BAND, VARIANT_LEAN, VARIANT_CLUSTER]
+        variants = [VARIANT_RING, VARIANT_BAND, VARIANT_LEAN, VARIANT_CLUSTER, VARIANT_PACKED]
     elif what == "cluster":   # where the lattice fits a cluster's shared memory: L = 1024, 2048, 4096
         shapes = [(1, 1024, 3.8, 100, 300), (1, 2048, 3.8, 100, 300), (1, 4096, 3.8, 100, 200), (1, 4096, 3.7446, 1000, 200),
                   (16, 2048, 3.7446, 2000, 200), (16, 2048, 3.8, 500, 200), (64, 1024, 3.75, 500, 200),
                   (9, 4096, 3.7446, 1000, 100), (16, 4096, 3.7446, 1000, 100), (64, 2048, 3.7446, 500, 100)]
         cases = [(fmt, B, L, r, warm, n) for (B, L, r, warm, n) in shapes for fmt in (FMT_U8, FMT_BITS)]
-        variants = [VARIANT_RING, VARIANT_LEAN, VARIANT_CLUSTER]
+        variants = [VARIANT_RING, VARIANT_LEAN, VARIANT_CLUSTER, VARIANT_PACKED]
     else:
         raise SystemExit(__doc__)
     table(cases, variants)
