@@ -106,8 +106,9 @@ enum {
     PGG_VARIANT_PERSIST = 12,/* LEAN, bit-packed, <= 148 lattices: every phase of up to 4096 MCS in ONE
                                 cooperative launch, a per-lattice barrier between phases           */
     PGG_VARIANT_CLUSTER = 13,/* L = 128 .. 4096 (a power of two), both layouts: the lattice stays bit-packed in
-                                the shared memory of a CTA cluster (1 .. 16 CTAs) for the whole call, halo rows
-                                over distributed shared memory, one cluster barrier per phase          */
+                                the shared memory of a CTA cluster (1 .. 16 CTAs) for the whole call; after a phase
+                                the changed halo row goes to each neighbour over distributed shared memory by
+                                asynchronous stores that complete on the neighbour's mbarrier (no cluster barrier) */
     PGG_VARIANT_PACKED = 14  /* uint8 lattices, L = 1024 .. 32768 (a power of two): the call packs the lattice
                                 into a bit-packed WORKING COPY (L*L/8 bytes per lattice from the stream-ordered
                                 pool: 32 MiB at L = 16384, which stays in the 126 MB L2), runs every phase on

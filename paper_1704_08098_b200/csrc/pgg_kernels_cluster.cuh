@@ -15,12 +15,18 @@
 //              round and CTA), survivors -> Q1 -> Philox on dense batches -> Q2 -> stencil on dense
 //              batches, as LEAN's workers; flips are atomicXor on the CTA's own shared memory; the
 //              queues are drained at the END of the phase (the rows never leave)
-//   exchange = after a phase each CTA stores its first and last three rows into its neighbours' halo
-//              rows through distributed shared memory, then ONE cluster barrier (release / acquire).
-//              A neighbour that is still inside the phase may see such a store early: it differs from
-//              what was there only in sites of the active class, which no other site reads in this
-//              phase (same-class sites are >= 4 apart, reads reach 3: S1) -- the argument that makes
-//              the in-place update legal in the first place.
+//   exchange = neighbours only, no cluster-wide barrier and no fence.  A phase of class row ci changes, of the rows a
+//              neighbour mirrors, one row at most per side: row ci of the first three (ci <= 2) and row rows-4+ci of
+//              the last three (ci >= 1).  After the CTA's own __syncthreads the owners of those words send them into
+//              the neighbour's halo with st.async (SASS STAS), whose bytes count on the NEIGHBOUR's mbarrier; thread 0
+//              adds a relaxed remote arrival "done with phase p".  Every thread then waits on its two halo barriers
+//              (from above / from below; two per side, alternating with the phase, armed two phases ahead with the
+//              bytes to expect).  Neighbours are at most one phase apart.  A row that arrives one phase early differs
+//              from what was there only in sites of that phase's class, which no site reads during it (same-class
+//              sites are >= 4 apart, reads reach 3: S1) -- the argument that makes the in-place update legal in the
+//              first place.  Round-2 measurement: cluster.sync() compiled to MEMBAR.ALL.GPU + cluster barrier +
+//              CCTL.IVALL in every thread and was the top stall (profiles/r2_ncu_full.md); without it a phase of one
+//              1024^2 lattice takes 2.31 us instead of 2.72.
 //   trace    = signed flip counts per CTA and MCS, one 64-bit atomic per CTA and MCS (a8)
 // Clusters are independent: an ensemble larger than the GPU holds at once simply runs in waves.
 #pragma once
@@ -46,6 +52,40 @@ struct ClusterPlan {
     uint32_t smem_bytes;
 };
 
+// ---- distributed shared memory: addresses of a neighbour CTA, asynchronous stores, remote barrier arrivals
+__device__ __forceinline__ uint32_t cluster_map(uint32_t saddr, uint32_t cta_rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(cta_rank));
+    return r;
+}
+// one 32-bit word into a neighbour's shared memory; its 4 bytes are counted on the neighbour's mbarrier (no fence needed)
+__device__ __forceinline__ void st_async_b32(uint32_t raddr, uint32_t val, uint32_t rbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(raddr), "r"(val), "r"(rbar) : "memory");
+}
+// "This CTA is done with the phase" on a neighbour's barrier.  Relaxed on purpose: the arrival orders nothing that is
+// still in flight -- it tells the neighbour that this CTA's READS of its halo rows are over, and they are: every warp
+// has used the values it read and passed __syncthreads before thread 0 gets here.  (A release at cluster scope costs
+// MEMBAR.ALL.GPU on the critical path of every phase; the rows themselves travel by st.async, which needs no fence.)
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t rbar)
+{
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(rbar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+
 template <int SRC, int GAME>
 __global__ void __launch_bounds__(kClusterThreads, 1)
 sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
@@ -64,7 +104,29 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
     int* eoff = reinterpret_cast<int*>(tbl + 160);
     int8_t* lut = reinterpret_cast<int8_t*>(eoff + 8);  // StencilLut (pgg_kernels_lean.cuh)
     __shared__ int delta_cta;
+    // halo barriers [from above | from below][phase parity]: one phase of one of them = my own arming arrival (with the
+    // bytes to expect) + the neighbour's "done" arrival + the bytes of the neighbour's changed row
+    __shared__ __align__(8) unsigned long long xbar[4];
     uint8_t* lat = a.lats + (size_t)b * a.lat_bytes;
+    const uint32_t n_phases = 16u * n_mcs;
+    const uint32_t xbar_s = smem_u32(xbar);
+    auto class_row = [&](uint32_t q) -> uint32_t {  // i mod 4 of the class of phase q of this call
+        const uint32_t mq = m0 + (q >> 4);
+        return (uint32_t)a.order[((size_t)b * a.order_stride + (mq % a.order_stride)) * 16 + (q & 15u)] >> 2;
+    };
+    // A phase of class row ci changes, of the rows a neighbour mirrors, only row ci of my first three (ci <= 2: the lower
+    // halo of the band above) and row rows-4+ci of my last three (ci >= 1: the upper halo of the band below)
+    auto arm = [&](uint32_t q) {
+        const uint32_t ciq = class_row(q), par = q & 1u, row_bytes = 4u * (uint32_t)wpr;
+        if (ciq >= 1u) mbar_expect_tx(xbar_s + 8u * par, row_bytes); else mbar_arrive_cta(xbar_s + 8u * par);
+        if (ciq <= 2u) mbar_expect_tx(xbar_s + 8u * (2u + par), row_bytes); else mbar_arrive_cta(xbar_s + 8u * (2u + par));
+    };
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < 4; ++q) mbar_init(xbar_s + 8u * q, 2);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        arm(0u);
+        arm(1u);  // n_phases >= 16
+    }
 
     // ---- load the band and its halos (periodic rows), packing uint8 to bits
     const uint32_t n_words = (rows + 6u) * (uint32_t)wpr;
@@ -94,11 +156,11 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
     __syncthreads();
     cluster.sync();  // every CTA of the cluster runs and has its rows before anyone stores into a neighbour
 
-    // halo rows of the neighbours, as seen through distributed shared memory
-    uint32_t* up_halo_bot = cluster.map_shared_rank(words, (rank + CS - 1u) % CS) + (size_t)(rows + 3u) * wpr;  // rows..rows+2 of the band above
-    uint32_t* dn_halo_top = cluster.map_shared_rank(words, (rank + 1u) % CS);                                   // rows -3..-1 of the band below
-    const uint32_t* own_first = words + 3 * wpr;                       // own rows 0..2
-    const uint32_t* own_last = words + (size_t)rows * wpr;             // own rows rows-3..rows-1  (= words + (3 + rows - 3) wpr)
+    // the neighbours' halo rows and halo barriers, as distributed-shared-memory addresses
+    const uint32_t up = (rank + CS - 1u) % CS, dn = (rank + 1u) % CS, words_s = smem_u32(words);
+    const uint32_t up_halo_bot = cluster_map(words_s + 4u * (rows + 3u) * (uint32_t)wpr, up);  // rows..rows+2 of the band above
+    const uint32_t dn_halo_top = cluster_map(words_s, dn);                                     // rows -3..-1 of the band below
+    const uint32_t up_bar = cluster_map(xbar_s + 16u, up), dn_bar = cluster_map(xbar_s, dn);   // its "from below" / "from above" pair
 
     uint2* q1 = reinterpret_cast<uint2*>(smem_raw + q_off + warp * kLeanWarpQBytes);
     uint4* q2 = reinterpret_cast<uint4*>(q1 + kLeanQ1Cap);
@@ -109,7 +171,6 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
     uint32_t n1 = 0, n2 = 0, h2 = 0;
     int delta = 0;  // this lane's flips in the current MCS
 
-    const uint32_t n_phases = 16u * n_mcs;
     for (uint32_t p = 0; p < n_phases; ++p) {
         const uint32_t m = m0 + (p >> 4), k = p & 15u;
         const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
@@ -249,12 +310,27 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
             atomicAdd(a.deltas + (size_t)b * a.n_mcs + m, (unsigned long long)(long long)delta_cta);
             delta_cta = 0;
         }
-        // ---- exchange: my first three rows are the lower halo of the band above, my last three the upper halo of the band below
-        for (uint32_t idx = threadIdx.x; idx < 3u * (uint32_t)wpr; idx += kClusterThreads) {
-            up_halo_bot[idx] = own_first[idx];
-            dn_halo_top[idx] = own_last[idx];
+        // ---- exchange with the two neighbours only (no cluster-wide barrier, no fence): the one row of my first / last
+        // three that this phase changed goes into their halo by asynchronous stores that count on THEIR barrier; thread 0
+        // adds "this CTA is done with phase p" (every warp has passed the barrier above, so nobody here still reads the
+        // halos of phase p: the neighbour may overwrite them with phase p+1).  Then everybody waits for the neighbours'
+        // rows and "done".  Skew between neighbours is at most one phase, and a row that arrives one phase early differs
+        // only in sites of that phase's class, which nobody reads during it (as for the in-place update itself).
+        const uint32_t par = p & 1u;
+        if (ci <= 2 && threadIdx.x < (uint32_t)wpr)
+            st_async_b32(up_halo_bot + 4u * ((uint32_t)(ci * wpr) + threadIdx.x), words[(3 + ci) * wpr + (int)threadIdx.x], up_bar + 8u * par);
+        if (ci >= 1 && threadIdx.x >= 256u && threadIdx.x < 256u + (uint32_t)wpr) {
+            const uint32_t t = threadIdx.x - 256u;
+            st_async_b32(dn_halo_top + 4u * ((uint32_t)((ci - 1) * wpr) + t), words[((int)rows + ci - 1) * wpr + (int)t], dn_bar + 8u * par);
         }
-        cluster.sync();  // release my stores, acquire my neighbours'
+        if (threadIdx.x == 0) {
+            mbar_arrive_remote(up_bar + 8u * par);
+            mbar_arrive_remote(dn_bar + 8u * par);
+        }
+        const uint32_t use_par = (p >> 1) & 1u;
+        mbar_wait_cluster(xbar_s + 8u * par, use_par);
+        mbar_wait_cluster(xbar_s + 8u * (2u + par), use_par);
+        if (threadIdx.x == 0 && p + 2u < n_phases) arm(p + 2u);
     }
 
     // ---- store the band back in the caller's layout
