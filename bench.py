@@ -357,6 +357,20 @@ def run_ours(args):
            "note": "achieved = updates/s x the time-averaged fraction of sites that need a draw "
                    "(pgg_count_interface at log-spaced MCS of the same run); peak = pgg_probe_draw_rate, "
                    "a kernel that makes STEP draws only (DESIGN.md section 5)"}
+    # instruction-issue view: warp instructions of one launch (ncu, profiles/traffic.json) over the measured launch time
+    # against what the SMs can issue (one warp instruction per cycle and scheduler, 4 schedulers per SM)
+    issue = None
+    try:
+        n_inst = json.loads(tr.read_text()).get(f"{'bits' if (packed or fmt == pgg.FMT_BITS) else 'u8'}_L{L}_warp_instructions_per_launch")
+        if n_inst and not dtile and clocks and clocks.get("sm_mhz"):
+            sms = torch.cuda.get_device_properties(local).multi_processor_count
+            peak_issue = sms * 4 * clocks["sm_mhz"] * 1e6
+            issue = {"warp_instructions_per_launch": n_inst, "achieved": n_inst / (phase_us * 1e-6) / 1e9,
+                     "peak": peak_issue / 1e9, "unit": "Gwarp-inst/s", "frac": n_inst / (phase_us * 1e-6) / peak_issue,
+                     "note": "ncu smsp__inst_executed.sum of one launch at MCS 600 / this run's average launch time; "
+                             "peak = SMs x 4 schedulers x the SM clock sampled during the timed region"}
+    except (ValueError, OSError):
+        pass
     if (fmt == pgg.FMT_BITS or packed) and not dtile:
         # the packed lattice is L2-resident: its bound is the integer pipes, not HBM
         alu.update({"traffic": roofline["traffic"], "kernel": roofline["kernel"], "avg_launch_us": phase_us,
@@ -374,6 +388,8 @@ def run_ours(args):
     else:
         roofline["alu_context"] = {k: alu[k] for k in ("achieved", "peak", "unit", "frac", "draw_fraction")}
 
+    if issue is not None:
+        roofline["issue_context"] = issue
     out = {
         "metric": METRIC, "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,

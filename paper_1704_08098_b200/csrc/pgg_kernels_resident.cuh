@@ -22,6 +22,7 @@
 //   may read the site itself.
 #pragma once
 #include "pgg_common.cuh"
+#include "pgg_stencil_lut.cuh"
 
 namespace pgg {
 
@@ -54,6 +55,7 @@ sweep_resident_kernel(PhaseArgs a, uint32_t m0, uint32_t n_chunk, ResPlan g)
     uint32_t* bits = res_smem;
     uint32_t* list = bits + g.n_words;            // (r << 16) | c of the sites that need a draw
     uint32_t* tbl = list + g.list_cap;
+    const int8_t* lut = reinterpret_cast<const int8_t*>(tbl + 160);  // StencilLut: the frame means no window ever wraps
     __shared__ uint32_t n_list[2];  // by phase parity: reset one while the other is in use
     __shared__ int s_delta[2];
 
@@ -80,6 +82,8 @@ sweep_resident_kernel(PhaseArgs a, uint32_t m0, uint32_t n_chunk, ResPlan g)
         bits[q] = w;
     }
     for (int q = tid; q < kTableSize; q += kResThreads) tbl[q] = a.tables[(size_t)b * kTableSize + q];
+    for (int q = tid; q < kStencilLutBytes / 4; q += kResThreads)
+        (tbl + 160)[q] = reinterpret_cast<const uint32_t*>(g_stencil_lut.v)[q];
     if (tid == 0) {
         n_list[0] = n_list[1] = 0u;
         s_delta[0] = s_delta[1] = 0;
@@ -162,13 +166,8 @@ sweep_resident_kernel(PhaseArgs a, uint32_t m0, uint32_t n_chunk, ResPlan g)
                 // bit offsets: e = step towards y, f = perpendicular step
                 const int ee = dir < 2u ? (dir == 0u ? -PB : PB) : (dir == 2u ? -1 : 1);
                 if (res_get(bits, off + ee) != sx) {
-                    const int f = dir < 2u ? 1 : PB, f2 = 2 * f;
-                    const int pm1 = off - ee, pm2 = pm1 - ee, p1 = off + ee, p2 = p1 + ee, p3 = p2 + ee;
-                    auto G = [&](int o) { return res_get(bits, o); };
-                    // A_x - A_y: weights of x's 13-site stencil minus those of y's (include/pgg.h)
-                    const int dA = G(pm2) + G(pm1) - G(p2) - G(p3) + 3 * (2 * sx - 1)
-                                 + 2 * (G(pm1 + f) + G(pm1 - f) - G(p2 + f) - G(p2 - f))
-                                 + G(off + f2) + G(off - f2) - G(p1 + f2) - G(p1 - f2);
+                    // A_x - A_y: six 7-bit windows (rows of the frame never wrap) index the weight table
+                    const int dA = bits_stencil_lut(off, dir, sx, bits, PW, lut);
                     if (u < tbl[sx * 102 + dA + 25]) {
                         // flip the site and its frame images
                         const int r2 = i < 3 ? r + L : (i >= L - 3 ? r - L : -1);
@@ -225,7 +224,7 @@ inline int resident_plan(int fmt, uint32_t L, ResPlan* p)
     p->PW = (L + 6 + 31) / 32;
     p->n_words = (L + 6) * p->PW;
     p->list_cap = (L / 4) * (L / 4);
-    p->smem_bytes = (p->n_words + p->list_cap + 160) * 4;
+    p->smem_bytes = (p->n_words + p->list_cap + 160) * 4 + kStencilLutBytes + 8;  // + 8: the window's second word after the last row
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(sweep_resident_kernel<kFmtU8>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
