@@ -601,6 +601,61 @@ def test_cluster_parity_sizes(fmt, L, n_mcs):
         assert_same(counts, ref_counts, f"counts L={L}")
 
 
+def test_packed_ensemble_init_and_continuation():
+    """PGG_VARIANT_PACKED (uint8 in HBM, bit-packed working copy for the length of the call): an ensemble that is
+    initialised inside the call, then continued by a second call from the uint8 state the first one left
+    (the working copy is private to a call), against the oracle; and the caller's buffer is the only output."""
+    L, B, fmt = 1024, 3, pgg.FMT_U8
+    use_variant(pgg.VARIANT_PACKED, fmt, L)
+    rs, seeds = [3.75, 3.9, 5.4], [2**40 + 1, 17, 99]
+    d = empty_lattice(fmt, L, B)
+    c1 = torch.zeros((B, 3), dtype=torch.int64, device="cuda")
+    c2 = torch.zeros((B, 2), dtype=torch.int64, device="cuda")
+    before = pgg.pgg_launch_count()
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, 3, c1)
+    # upload, init, density, pack, order, 16 phases per MCS, unpack, finalize
+    assert pgg.pgg_launch_count() - before == 1 + 1 + 1 + 1 + 1 + 16 * 3 + 1 + 1
+    assert pgg.pgg_get_variant_used() == pgg.VARIANT_PACKED
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_PERM, -1.0, 3, 2, c2)
+    torch.cuda.synchronize()
+    got = to_host(d, fmt, L)
+    for b in range(B):
+        ref = orc.init(L, 0.5, seeds[b])
+        r1, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, 3, n_threads=orc.max_threads())
+        r2, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_PERM, 3, 2, n_threads=orc.max_threads())
+        assert_same(got[b], ref, f"member {b}")
+        assert_same(c1[b].cpu().numpy().astype(np.uint64), r1, f"counts of call 1, member {b}")
+        assert_same(c2[b].cpu().numpy().astype(np.uint64), r2, f"counts of call 2, member {b}")
+    pgg.pgg_trim_workspace()  # gives the pool's cached working copy back; the next call allocates afresh
+    lat0 = got[0].copy()
+    ref = lat0.copy()
+    orc.sweep(ref, 3.8, K, 5, pgg.ORDER_IID, 5, 1, n_threads=orc.max_threads())
+    out, _ = gpu_sweep(lat0, fmt, 3.8, 5, pgg.ORDER_IID, 5, 1)
+    assert_same(out, ref, "after pgg_trim_workspace")
+
+
+@pytest.mark.parametrize("cs", [1, 2, 4, 8, 16])
+def test_cluster_every_cluster_size(cs, monkeypatch):
+    """The neighbour-only halo exchange (asynchronous stores that complete on the neighbour's mbarrier, no cluster
+    barrier) for every cluster size, CS = 1 (the CTA is its own neighbour) and CS = 2 (both neighbours are the same
+    CTA) included: five lattices of L = 512 for 50 MCS (800 phases, every class row many times) against the oracle."""
+    monkeypatch.setenv("PGG_CLUSTER_SIZE", str(cs))
+    L, B, n_mcs, fmt = 512, 5, 50, pgg.FMT_BITS
+    use_variant(pgg.VARIANT_CLUSTER, fmt, L)
+    rs = [3.74 + 0.02 * b for b in range(B)]
+    seeds = [2**36 + 11 * b + cs for b in range(B)]
+    d = empty_lattice(fmt, L, B)
+    cnt = torch.zeros((B, n_mcs), dtype=torch.int64, device="cuda")
+    pgg.pgg_run_ensemble(d, fmt, B, L, rs, K, seeds, pgg.ORDER_IID, 0.5, 0, n_mcs, cnt)
+    torch.cuda.synchronize()
+    got = to_host(d, fmt, L)
+    for b in range(B):
+        ref = orc.init(L, 0.5, seeds[b])
+        ref_counts, _ = orc.sweep(ref, rs[b], K, seeds[b], pgg.ORDER_IID, 0, n_mcs, n_threads=orc.max_threads())
+        assert_same(got[b], ref, f"member {b}, cluster size {cs}")
+        assert_same(cnt[b].cpu().numpy().astype(np.uint64), ref_counts, f"counts of member {b}, cluster size {cs}")
+
+
 @pytest.mark.parametrize("fmt", FMTS)
 def test_cluster_structured_ensembles_and_waves(fmt):
     """Structured and absorbing states; an ensemble of 40 lattices of L = 1024 (more clusters than the GPU
