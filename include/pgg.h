@@ -104,7 +104,7 @@ enum {
     PGG_VARIANT_LEAN = 11,   /* L = 1024 .. 32768, a power of two: whole rows streamed, packed to
                                 bits on arrival (uint8), scan / draw / stencil on a bit ring   */
     PGG_VARIANT_PERSIST = 12,/* LEAN, bit-packed, <= 148 lattices: every phase of up to 4096 MCS in ONE
-                                cooperative launch, a per-lattice barrier between phases           */
+                                cooperative launch; between phases a band waits for its two neighbour bands only */
     PGG_VARIANT_CLUSTER = 13,/* L = 128 .. 4096 (a power of two), both layouts: the lattice stays bit-packed in
                                 the shared memory of a CTA cluster (1 .. 16 CTAs) for the whole call; after a phase
                                 the changed halo row goes to each neighbour over distributed shared memory by

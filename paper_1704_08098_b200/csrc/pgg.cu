@@ -389,8 +389,9 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
         if (rc != 0) return fail(PGG_ERR_CUDA, "cluster kernel setup failed: %s", cudaGetErrorString((cudaError_t)rc));
     }
     unsigned int* d_gbar = nullptr;
+    const size_t gbar_bytes = sizeof(unsigned int) * (size_t)B * 160;  // one flag per band: nb <= SMs / B, at least 1
     if (variant == PGG_VARIANT_PERSIST) {
-        PGG_CUDA(tmp.alloc((void**)&d_gbar, sizeof(unsigned int) * B));
+        PGG_CUDA(tmp.alloc((void**)&d_gbar, gbar_bytes));
     }
     if (variant == PGG_VARIANT_LEAN || variant == PGG_VARIANT_PERSIST) {
         int32_t rc = pgg::lean_plan(kfmt, L, B, &lplan);
@@ -417,7 +418,7 @@ int32_t run_sweeps(uint8_t* d_lats, int32_t fmt, uint32_t B, uint32_t L, const d
             continue;
         }
         if (variant == PGG_VARIANT_PERSIST) {   // likewise, cooperative: a barrier per phase instead of a launch
-            PGG_CUDA(cudaMemsetAsync(d_gbar, 0, sizeof(unsigned int) * B, stream));
+            PGG_CUDA(cudaMemsetAsync(d_gbar, 0, gbar_bytes, stream));
             PGG_CUDA(pgg::lean_persist_launch(lplan, a, m0, n_chunk, B, d_gbar, stream, game));
             PGG_LAUNCHED();
             continue;

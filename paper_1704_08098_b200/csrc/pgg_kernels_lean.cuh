@@ -124,7 +124,7 @@ __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar)
 // the mbarriers are initialised afresh, which is legal because every warp has passed the closing
 // __syncthreads of the previous phase).
 template <int SRC, int GAME, bool PERSIST>
-__device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint32_t k, const LeanPlan& g)
+__device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint32_t k, const LeanPlan& g, bool tables = true)
 {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int pitch = (int)g.pitch, RC = (int)g.RC;
@@ -149,11 +149,13 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
     const uint32_t bar_sfull = bar_empty + 8u * kLeanMaxSlots, bar_sempty = bar_sfull + 8u * kLeanMaxSlots;  // of the staging slots
 
     if (!PERSIST) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    for (int q = threadIdx.x; q < kTableSize; q += blockDim.x)
-        tbl[q] = a.tables[(size_t)b * kTableSize + q];
-    if (GAME == kGamePGG)
-        for (int q = threadIdx.x; q < kStencilLutBytes / 4; q += blockDim.x)
-            reinterpret_cast<uint32_t*>(lut)[q] = reinterpret_cast<const uint32_t*>(g_stencil_lut.v)[q];
+    if (tables) {  // (PERSIST: shared memory keeps them from phase to phase)
+        for (int q = threadIdx.x; q < kTableSize; q += blockDim.x)
+            tbl[q] = a.tables[(size_t)b * kTableSize + q];
+        if (GAME == kGamePGG)
+            for (int q = threadIdx.x; q < kStencilLutBytes / 4; q += blockDim.x)
+                reinterpret_cast<uint32_t*>(lut)[q] = reinterpret_cast<const uint32_t*>(g_stencil_lut.v)[q];
+    }
     if (threadIdx.x == 0) {
         delta_cta = 0;
         for (uint32_t s = 0; s < NR; ++s) {
@@ -486,31 +488,41 @@ phase_lean_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g)
 // ---------------------------------------------------------------------------
 // PERSIST: every phase of n_mcs MCS (16 n_mcs phases) in ONE cooperative launch, bit-packed source.
 // ("minimizing the need to access global memory" -- and, on this machine, the launches.)
-// The lattice stays where it is (L2-resident for the sizes this is used for); between two phases the
-// CTAs of one lattice meet at a barrier in global memory -- lattices of an ensemble never wait for
-// each other.  A phase reads what the previous one wrote within radius 3 of every site, so the
-// barrier is the method's own dependency, not an artefact; what it saves is the launch, the drain of
-// the grid and the refill of 148 empty pipelines behind a grid-wide dependency.
-// gbar[b] counts arrivals of lattice b's CTAs (zeroed by the host); after phase p it reaches (p+1) nb.
+// The lattice stays where it is (L2-resident for the sizes this is used for).  A phase reads what the previous
+// one wrote within radius 3 of every site, so a band (whole rows) waits, between two phases, for its TWO
+// NEIGHBOUR bands only -- a flag per band in global memory, release / acquire at GPU scope; no grid-wide barrier,
+// lattices of an ensemble never wait for each other.  What it saves is the launch, the drain of the grid and the
+// refill of 148 empty pipelines behind a grid-wide dependency; what it costs is the flag round trip through L2
+// and the set-up of a phase on the critical path (a dependent launch hides its set-up behind the previous
+// phase's tail) -- measured slower than the launches (DESIGN.md appendix B): selectable, never AUTO.
+// gbar[b * nb + band] = phases band `band` of lattice b has completed (zeroed by the host).
 // ---------------------------------------------------------------------------
 template <int GAME>
 __global__ void __launch_bounds__(kLeanThreads, 1)
 sweep_lean_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, LeanPlan g, unsigned int* __restrict__ gbar)
 {
     const uint32_t n_phases = 16u * n_mcs;
-    unsigned int* bar = gbar + blockIdx.y;
+    // done[band] = phases this band has completed.  A band reads its neighbours' three nearest rows and nothing
+    // further, so phase p + 1 of band b needs phase p of bands b - 1, b, b + 1 only (both ways: they must also be
+    // done READING b's rows of phase p before b changes them): neighbours are at most one phase apart, the rest
+    // of the lattice may drift -- no grid-wide barrier, a slow band delays only its neighbourhood.
+    unsigned int* done = gbar + (size_t)blockIdx.y * g.nb;
+    const uint32_t band = blockIdx.x;
+    const unsigned int* up = done + (band + g.nb - 1u) % g.nb;
+    const unsigned int* dn = done + (band + 1u) % g.nb;
     for (uint32_t p = 0; p < n_phases; ++p) {
-        lean_phase<kFmtBits, GAME, true>(a, m0 + (p >> 4), p & 15u, g);  // ends with __syncthreads()
+        lean_phase<kFmtBits, GAME, true>(a, m0 + (p >> 4), p & 15u, g, p == 0);  // ends with __syncthreads()
         if (p + 1 == n_phases) break;
         if (threadIdx.x == 0) {
-            __threadfence();  // this CTA's flips (atomics) and counts before its arrival
-            atomicAdd(bar, 1u);
-            const unsigned int target = (p + 1u) * g.nb;
-            unsigned int seen, spins = 0;
+            __threadfence();  // this CTA's flips (atomics) and counts before its flag
+            const unsigned int target = p + 1u;
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + band), "r"(target) : "memory");
+            unsigned int s0, s1, spins = 0;
             for (;;) {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
-                if (seen >= target) break;
-                __nanosleep(40);
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(s0) : "l"(up) : "memory");
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(s1) : "l"(dn) : "memory");
+                if (s0 >= target && s1 >= target) break;
+                __nanosleep(20);
                 if (++spins > (1u << 24)) __trap();  // ~1 s: a lost CTA must not hang the device
             }
         }
