@@ -86,7 +86,8 @@ enum { PGG_ORDER_IID = 0, PGG_ORDER_PERM = 1, PGG_ORDER_DTILE = 2 };
  * ladder kept for comparison: selectable, tested, never chosen.  Tuning knobs read from the environment by
  * the plan functions (defaults are the measured best; every setting is bit-exact): PGG_PDL,
  * PGG_RING_{SLOTS,L2PF,FULLROW,TPR_LOG2,MIRROR,ROTATE}, PGG_BAND_SLOTS, PGG_DYN_WARPS, PGG_PIPE_STAGES,
- * PGG_TILE_{CTAS_PER_SM,STAGES}, PGG_LEAN_{LAG,AHEAD,SLOT_ROWS,SLOTS,WORDS}, PGG_CLUSTER_SIZE.            */
+ * PGG_TILE_{CTAS_PER_SM,STAGES}, PGG_LEAN_{LAG,AHEAD,SLOT_ROWS,SLOTS,WORDS}, PGG_CLUSTER_SIZE, and
+ * PGG_PACKED_MIN_L (the smallest uint8 L for which AUTO takes PACKED; read once per process).             */
 enum {
     PGG_VARIANT_AUTO = 0,
     PGG_VARIANT_V0 = 1,   /* one thread per active site, global loads, any L % 4 == 0 */

@@ -92,6 +92,19 @@ def test_argument_validation_returns_error_codes():
     assert h.pgg_run_ensemble(fake, 0, 1, 64, None, 0.5, s, 0, 0.5, 0, 1, None, None) == pgg.ERR_NULL
     assert h.pgg_set_variant(99) == pgg.ERR_UNSUPPORTED
     assert b"variant" in h.pgg_last_error()
+    # pgg_sweep_static: pgg_sweep's checks, its own limit (PGG_STATIC_MAX_MCS), no double-tiling schedule; all of
+    # them before the first CUDA call, and n_mcs == 0 is a no-op that touches nothing
+    assert h.pgg_sweep_static(None, 0, 64, 4.0, 0.5, 1, 0, 0, 1, None, None) == pgg.ERR_NULL
+    assert h.pgg_sweep_static(fake, 0, 6, 4.0, 0.5, 1, 0, 0, 1, None, None) == pgg.ERR_BAD_L
+    assert h.pgg_sweep_static(fake + 4, 0, 64, 4.0, 0.5, 1, 0, 0, 1, None, None) == pgg.ERR_ALIGN
+    assert h.pgg_sweep_static(fake, 0, 64, 4.0, 0.0, 1, 0, 0, 1, None, None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_sweep_static(fake, 0, 64, float("nan"), 0.5, 1, 0, 0, 1, None, None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_sweep_static(fake, 0, 64, 4.0, 0.5, 1, 0, 2**32 - 1, 2, None, None) == pgg.ERR_BAD_PARAM
+    assert h.pgg_sweep_static(fake, 0, 64, 4.0, 0.5, 1, pgg.ORDER_DTILE, 0, 1, None, None) == pgg.ERR_UNSUPPORTED
+    assert h.pgg_sweep_static(fake, 0, 64, 4.0, 0.5, 1, 9, 0, 1, None, None) == pgg.ERR_UNSUPPORTED
+    assert h.pgg_sweep_static(fake, 0, 64, 4.0, 0.5, 1, 0, 0, pgg.STATIC_MAX_MCS + 1, None, None) == pgg.ERR_BAD_PARAM
+    assert b"PGG_STATIC_MAX_MCS" in h.pgg_last_error()
+    assert h.pgg_sweep_static(fake, 0, 64, 4.0, 0.5, 1, 0, 0, 0, None, None) == pgg.OK
     with pytest.raises(pgg.PggError):
         pgg.pgg_build_accept_table(4.0, -1.0)
 
