@@ -137,3 +137,30 @@ def test_static_sweep_at_the_limit():
     pgg.pgg_sweep_static(y, fmt, L, 3.8, K, 9, pgg.ORDER_IID, 0, n, cy)
     torch.cuda.synchronize()
     assert torch.equal(x, y) and torch.equal(cx, cy)
+
+
+@pytest.mark.parametrize("fmt,L,kernel", [(f, L, k) for f, L, k, _, _ in CASES])
+def test_static_sweep_is_capturable_into_a_cuda_graph(fmt, L, kernel):
+    """What the entry point is for: the whole call (memsets, the upload / order / density / phase / finalize kernels,
+    cluster and programmatic-dependent launches) is captured into a CUDA graph -- an allocation would fail the
+    capture -- and two replays equal two eager pgg_sweep calls bit for bit.  One warm-up call outside the capture
+    resolves the scratch address and the function attributes."""
+    n = 3
+    a = to_device(wl.random_lattice(L, 0.5, 31), fmt)
+    b = a.clone()
+    ca = torch.zeros(n, dtype=torch.int64, device="cuda")
+    cb = torch.zeros(n, dtype=torch.int64, device="cuda")
+    for _ in range(2):
+        pgg.pgg_sweep(a, fmt, L, 3.8, K, 3, pgg.ORDER_IID, 0, n, ca)
+    warm = b.clone()
+    pgg.pgg_sweep_static(warm, fmt, L, 3.8, K, 3, pgg.ORDER_IID, 0, 1)
+    assert pgg.pgg_get_variant_used() == kernel
+    torch.cuda.synchronize()
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            pgg.pgg_sweep_static(b, fmt, L, 3.8, K, 3, pgg.ORDER_IID, 0, n, cb, stream=side)
+    graph.replay()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(a, b) and torch.equal(ca, cb)
