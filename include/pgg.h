@@ -32,8 +32,11 @@
  * exception and says so): per-lattice parameters reach the device as kernel arguments, not by
  * copies from pageable memory, so host arrays may be freed on return.  Results are valid once
  * the caller has synchronised the stream.  The kernel-variant switch (pgg_set_variant) and the
- * environment knobs DESIGN.md lists are process-wide; a call uses the current CUDA device.  Temporary device memory is taken and returned
- * with the stream-ordered allocator (cudaMallocAsync / cudaFreeAsync).
+ * environment knobs DESIGN.md lists are process-wide; a call uses the current CUDA device.
+ * Temporary device memory (seeds, tables, class order, the working copy of PGG_VARIANT_PACKED) is taken
+ * from and returned to a stream-ordered memory pool the library owns, one per device
+ * (cudaMallocFromPoolAsync / cudaFreeAsync; pgg_trim_workspace() gives it back to the driver);
+ * pgg_sweep_static takes none at all.
  */
 #ifndef PGG_H_
 #define PGG_H_
