@@ -408,11 +408,13 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
             const uint32_t excl = __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt) + 8u * __popc(b3 & lt);
             uint2* dst = q1 + n1 + excl;
             while (z) {  // two survivors per trip: the highest and the lowest set bit
-                const uint32_t hi = 31u - (uint32_t)__clz(z), lo = (uint32_t)__ffs((int)z) - 1u;
+                uint32_t hi;  // bfind = the position of the highest set bit (one FLO; 31 - __clz costs three)
+                asm("bfind.u32 %0, %1;" : "=r"(hi) : "r"(z));
+                const uint32_t lo = (uint32_t)__ffs((int)z) - 1u;
                 dst[0] = make_uint2(xb + hi, sb + hi);
                 if (hi != lo) dst[1] = make_uint2(xb + lo, sb + lo);
                 dst += 2;  // (a lone last survivor leaves dst one too far: it is not used again)
-                z &= ~((1u << hi) | (1u << lo));
+                z = (z & (z - 1u)) & ~(1u << hi);  // drop the lowest and the highest set bit
             }
             __syncwarp();
             n1 += tot;
