@@ -258,8 +258,7 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
         };
         auto extract_round = [&](uint32_t z, uint32_t xb, uint32_t sb, bool may_split) {
             const uint32_t cnt = __popc(z);
-            const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, cnt & 1u), b1 = __ballot_sync(0xFFFFFFFFu, cnt & 2u);
-            const uint32_t b2 = __ballot_sync(0xFFFFFFFFu, cnt & 4u), b3 = __ballot_sync(0xFFFFFFFFu, cnt & 8u);
+            const uint32_t b0 = ballot_bit<0>(cnt), b1 = ballot_bit<1>(cnt), b2 = ballot_bit<2>(cnt), b3 = ballot_bit<3>(cnt);
             const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, cnt);  // one REDUX instead of four POPC and three adds
             if (may_split && tot > 128u) return false;
             const uint32_t excl = __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt) + 8u * __popc(b3 & lt);

@@ -95,6 +95,22 @@ __device__ __forceinline__ uint32_t lean_pack16(uint4 v)
     return (a & 0xFFu) | (b2 & ~0xFFu);                // bits 0..7 | bits 8..15 (| junk above)
 }
 
+// Ballot of bit `BIT` of v over the full warp.  (and + setp.ne in PTX become one LOP3 that writes the predicate;
+// the C++ form compiled to a shift, an and and a compare per ballot.)
+template <int BIT>
+__device__ __forceinline__ uint32_t ballot_bit(uint32_t v)
+{
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b32 t;\n\t"
+        "and.b32 t, %1, %2;\n\t"
+        "setp.ne.u32 p, t, 0;\n\t"
+        "vote.sync.ballot.b32 %0, p, 0xffffffff;\n\t}"
+        : "=r"(r)
+        : "r"(v), "n"(1u << BIT));
+    return r;
+}
+
 // The producer's wait: it has a whole step of slack, so it backs off instead of competing for issue slots.
 __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity)
 {
@@ -401,8 +417,7 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
             // prefix sum of the per-lane counts (0..8) from four ballots: the bits of the counts are summed
             // by population counts, all independent -- a shuffle scan is five dependent round trips
             const uint32_t cnt = __popc(z);
-            const uint32_t b0 = __ballot_sync(0xFFFFFFFFu, cnt & 1u), b1 = __ballot_sync(0xFFFFFFFFu, cnt & 2u);
-            const uint32_t b2 = __ballot_sync(0xFFFFFFFFu, cnt & 4u), b3 = __ballot_sync(0xFFFFFFFFu, cnt & 8u);
+            const uint32_t b0 = ballot_bit<0>(cnt), b1 = ballot_bit<1>(cnt), b2 = ballot_bit<2>(cnt), b3 = ballot_bit<3>(cnt);
             const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, cnt);  // one REDUX instead of four POPC and three adds
             if (may_split && tot > 128u) return false;
             const uint32_t excl = __popc(b0 & lt) + 2u * __popc(b1 & lt) + 4u * __popc(b2 & lt) + 8u * __popc(b3 & lt);
