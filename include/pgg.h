@@ -220,6 +220,60 @@ int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, d
                      uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t n_mcs, uint64_t* d_counts,
                      void* stream);
 
+/* ---- One lattice sharded over several GPUs as ROW SLABS (the periodic L x L lattice
+ * is PAPER.md:45, the step PAPER.md:58-60).  One process per GPU holds lattice rows [row0, row0 + n_rows)
+ * plus three halo rows on either side -- the read stencil of a step has radius 3:
+ *   d_slab : (n_rows + 6) whole rows in layout fmt (pgg_slab_bytes), 16-byte aligned; buffer row q holds
+ *            lattice row (row0 - 3 + q) mod L.  The caller fills own rows AND halo rows once, before the
+ *            first phase; after that the library keeps the halos current.
+ *   row0 % 4 == 0, n_rows % 4 == 0, n_rows >= 4, row0 + n_rows <= L.
+ * pgg_slab_sweep runs n_phases consecutive phases of the 16-sublattice schedule on the slab's own rows,
+ * starting at phase k_begin (0..15) of MCS t_begin and running on into the following MCS.  The Philox
+ * counter carries the site index of the WHOLE lattice, so the slabs together evolve bit for bit as
+ * pgg_sweep evolves the unsharded lattice (r, K, seed, order_mode as there; PGG_ORDER_IID / _PERM only).
+ * Halo push, fused into the phase kernel: a thread that flips a site of the slab's first (last) three own
+ * rows also stores the new value through d_up_halo (d_dn_halo):
+ *   d_up_halo : three rows, layout fmt -- the upper neighbour's copy of this slab's own rows 0..2, i.e. rows
+ *               n_rows' + 3 .. n_rows' + 5 of ITS buffer (n_rows' = its row count);
+ *   d_dn_halo : three rows -- the lower neighbour's copy of own rows n_rows-3 .. n_rows-1 = rows 0..2 of its buffer.
+ *   Both are plain device pointers: memory of this GPU (several slabs on one device; a single slab is its own
+ *   neighbour both ways) or of a peer GPU (pgg_slab_ipc_open; stores and 32-bit atomics over NVLink P2P).
+ * Order between phases.  Phase p + 1 of a slab needs phase p of its two neighbours complete (their pushes
+ * landed; and they have finished reading what p + 1 overwrites).  Two ways:
+ *   d_flags == NULL : the caller orders the launches (slabs of one device driven phase by phase on one stream).
+ *   d_flags != NULL : three uint32 on THIS device (zero before epoch 0): [0] internal, [1] / [2] = phases the
+ *               upper / lower neighbour has completed.  d_up_flag = address of the upper neighbour's
+ *               flags[2], d_dn_flag = address of the lower neighbour's flags[1] (local or peer memory).  The
+ *               phase with global number e = epoch0 + p starts when flags[1] >= e and flags[2] >= e (acquire,
+ *               system scope; a wait of seconds traps instead of hanging) and, complete, stores e + 1 to both
+ *               neighbours (release, system scope).  All slabs of the lattice must run the same phases with the
+ *               same epoch numbers; epoch0 continues from call to call.  No host synchronisation, no NCCL on
+ *               the data path: neighbouring slabs are at most one phase apart.
+ *   d_deltas : NULL or device array of uint64 (two's complement), one per MCS the call touches
+ *               (ceil((k_begin + n_phases) / 16)): the signed number of flips of this slab's own rows in MCS
+ *               t_begin + m is ADDED to d_deltas[m].  The rho_C trace (Eq. 4) is the initial count
+ *               plus the running sum of the deltas summed over all slabs (one all-reduce per call, not per phase).
+ * At most PGG_SLAB_MAX_MCS MCS per call.  The kernel is V0's (one thread per active site).
+ * Errors: PGG_ERR_NULL, PGG_ERR_BAD_L, PGG_ERR_ALIGN, PGG_ERR_BAD_PARAM (rows, k_begin, r, K, span, epochs),
+ * PGG_ERR_UNSUPPORTED (fmt, order_mode), PGG_ERR_CUDA.  n_phases == 0 is a no-op.
+ * pgg_slab_alloc / pgg_slab_free: cudaMalloc'ed, zeroed memory of its own allocation (what an IPC handle
+ * needs; torch tensors are carved out of larger blocks) -- both synchronise the device.
+ * pgg_slab_ipc_export: 64-byte handle of such an allocation, to be sent to the neighbour processes;
+ * pgg_slab_ipc_open: the neighbour's allocation mapped into this process (peer_device = the CUDA ordinal it
+ * lives on, or -1 if unknown / the same device; PGG_ERR_UNSUPPORTED without a P2P path); pgg_slab_ipc_close. */
+#define PGG_SLAB_MAX_MCS 4096u
+#define PGG_SLAB_IPC_HANDLE_BYTES 64
+uint64_t pgg_slab_bytes(int32_t fmt, uint32_t L, uint32_t n_rows);
+int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
+                       uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
+                       void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,
+                       uint32_t epoch0, uint64_t* d_deltas, void* stream);
+int32_t pgg_slab_alloc(uint64_t bytes, void** d_out);
+int32_t pgg_slab_free(void* d_ptr);
+int32_t pgg_slab_ipc_export(void* d_ptr, uint8_t* h_handle64);
+int32_t pgg_slab_ipc_open(const uint8_t* h_handle64, int32_t peer_device, void** d_out);
+int32_t pgg_slab_ipc_close(void* d_ptr);
+
 /* The 16 phase classes of MCS t, computed by the library's own
  * device kernel and copied back; h_out16: host array of 16 bytes.  Synchronises
  * `stream`.  For tests of step a1.  PGG_ORDER_DTILE has no classes:

@@ -43,6 +43,15 @@ SIGNATURES = {
     "pgg_pd_build_accept_table": (C.c_int32, [C.c_double] * 5 + [_u32p]),
     "pgg_pd_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32] + [C.c_double] * 5 +
                      [C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]),
+    "pgg_slab_bytes": (C.c_uint64, [C.c_int32, C.c_uint32, C.c_uint32]),
+    "pgg_slab_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_double, C.c_double,
+                                   C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p,
+                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]),
+    "pgg_slab_alloc": (C.c_int32, [C.c_uint64, C.POINTER(C.c_void_p)]),
+    "pgg_slab_free": (C.c_int32, [C.c_void_p]),
+    "pgg_slab_ipc_export": (C.c_int32, [C.c_void_p, _u8p]),
+    "pgg_slab_ipc_open": (C.c_int32, [_u8p, C.c_int32, C.POINTER(C.c_void_p)]),
+    "pgg_slab_ipc_close": (C.c_int32, [C.c_void_p]),
     "pgg_phase_classes": (C.c_int32, [C.c_uint64, C.c_uint32, C.c_int32, _u8p, C.c_void_p]),
     "pgg_set_variant": (C.c_int32, [C.c_int32]),
     "pgg_get_variant_used": (C.c_int32, []),
@@ -92,7 +101,8 @@ def _stream(stream) -> int:
 
 
 def _ptr(t) -> int:
-    return 0 if t is None else t.data_ptr()
+    """Device address: a tensor, an int (an address from pgg_slab_alloc / pgg_slab_ipc_open) or None."""
+    return 0 if t is None else t if isinstance(t, int) else t.data_ptr()
 
 
 def pgg_build_accept_table(r: float, K: float):
@@ -146,6 +156,51 @@ def pgg_pd_sweep(d_lat, fmt: int, L: int, R: float, S: float, T: float, P: float
                  order_mode: int, t_begin: int, n_mcs: int, d_counts=None, stream=None) -> None:
     _check(lib().pgg_pd_sweep(_ptr(d_lat), fmt, L, R, S, T, P, K, seed, order_mode, t_begin, n_mcs,
                               _ptr(d_counts), _stream(stream)))
+
+
+SLAB_MAX_MCS = 4096  # PGG_SLAB_MAX_MCS
+SLAB_IPC_HANDLE_BYTES = 64
+
+
+def pgg_slab_bytes(fmt: int, L: int, n_rows: int) -> int:
+    return int(lib().pgg_slab_bytes(fmt, L, n_rows))
+
+
+def pgg_slab_sweep(d_slab, fmt: int, L: int, row0: int, n_rows: int, r: float, K: float, seed: int, order_mode: int,
+                   t_begin: int, k_begin: int, n_phases: int, d_up_halo, d_dn_halo, d_flags=None, d_up_flag=None,
+                   d_dn_flag=None, epoch0: int = 0, d_deltas=None, stream=None) -> None:
+    """n_phases phases on one row slab of a sharded lattice (include/pgg.h); pointers are tensors or addresses."""
+    _check(lib().pgg_slab_sweep(_ptr(d_slab), fmt, L, row0, n_rows, r, K, seed, order_mode, t_begin, k_begin, n_phases,
+                                _ptr(d_up_halo), _ptr(d_dn_halo), _ptr(d_flags), _ptr(d_up_flag), _ptr(d_dn_flag),
+                                epoch0, _ptr(d_deltas), _stream(stream)))
+
+
+def pgg_slab_alloc(n_bytes: int) -> int:
+    """-> device address of a zeroed cudaMalloc allocation of its own (exportable by pgg_slab_ipc_export)."""
+    p = C.c_void_p(0)
+    _check(lib().pgg_slab_alloc(n_bytes, C.byref(p)))
+    return int(p.value)
+
+
+def pgg_slab_free(d_ptr: int) -> None:
+    _check(lib().pgg_slab_free(d_ptr))
+
+
+def pgg_slab_ipc_export(d_ptr: int) -> bytes:
+    h = (C.c_uint8 * SLAB_IPC_HANDLE_BYTES)()
+    _check(lib().pgg_slab_ipc_export(d_ptr, h))
+    return bytes(h)
+
+
+def pgg_slab_ipc_open(handle: bytes, peer_device: int = -1) -> int:
+    h = (C.c_uint8 * SLAB_IPC_HANDLE_BYTES)(*handle)
+    p = C.c_void_p(0)
+    _check(lib().pgg_slab_ipc_open(h, peer_device, C.byref(p)))
+    return int(p.value)
+
+
+def pgg_slab_ipc_close(d_ptr: int) -> None:
+    _check(lib().pgg_slab_ipc_close(d_ptr))
 
 
 def pgg_phase_classes(seed: int, t: int, order_mode: int, stream=None):

@@ -27,6 +27,7 @@
 #include "pgg_kernels_cluster.cuh"
 #include "pgg_kernels_dtile.cuh"
 #include "pgg_kernels_probe.cuh"
+#include "pgg_kernels_slab.cuh"
 
 namespace {
 
@@ -802,6 +803,145 @@ int32_t pgg_count_interface(const void* d_lat, int32_t fmt, uint32_t L, uint64_t
         pgg::interface_count_kernel<pgg::kFmtBits><<<grid, 256, 0, s>>>(static_cast<const uint8_t*>(d_lat), L,
                                                                       reinterpret_cast<unsigned long long*>(d_count));
     PGG_LAUNCHED();
+    return PGG_OK;
+}
+
+// ---- row slabs of one lattice over several GPUs (kernels in pgg_kernels_slab.cuh) ----
+
+uint64_t pgg_slab_bytes(int32_t fmt, uint32_t L, uint32_t n_rows)
+{
+    const unsigned long long row = fmt == PGG_FMT_U8 ? L : L / 8;
+    return row * ((unsigned long long)n_rows + 6ull);
+}
+
+int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
+                       uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
+                       void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,
+                       uint32_t epoch0, uint64_t* d_deltas, void* stream_)
+{
+    int32_t rc = check_lattice_args(d_slab, fmt, L);
+    if (rc != PGG_OK) return rc;
+    if (d_up_halo == nullptr || d_dn_halo == nullptr) return fail(PGG_ERR_NULL, "halo pointer is NULL");
+    const uintptr_t align = fmt == PGG_FMT_BITS ? 3u : 0u;  // bit rows are updated by 32-bit atomics
+    if ((reinterpret_cast<uintptr_t>(d_up_halo) & align) || (reinterpret_cast<uintptr_t>(d_dn_halo) & align))
+        return fail(PGG_ERR_ALIGN, "bit-packed halo rows must be 4-byte aligned");
+    if (n_rows < 4 || n_rows % 4 != 0 || row0 % 4 != 0 || (unsigned long long)row0 + n_rows > L)
+        return fail(PGG_ERR_BAD_PARAM, "slab rows [%u, %u + %u): need row0 %% 4 == 0, n_rows %% 4 == 0, n_rows >= 4, row0 + n_rows <= L = %u",
+                    row0, row0, n_rows, L);
+    if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM)
+        return fail(PGG_ERR_UNSUPPORTED, "slabs run the 16-sublattice schedule only (PGG_ORDER_IID / PGG_ORDER_PERM), not order_mode %d", order_mode);
+    if (!(K > 0.0) || !std::isfinite(K)) return fail(PGG_ERR_BAD_PARAM, "K must be finite and > 0");
+    if (!std::isfinite(r)) return fail(PGG_ERR_BAD_PARAM, "r is not finite");
+    if (k_begin >= 16) return fail(PGG_ERR_BAD_PARAM, "k_begin = %u: a MCS has phases 0 .. 15", k_begin);
+    if (d_flags != nullptr && (d_up_flag == nullptr || d_dn_flag == nullptr))
+        return fail(PGG_ERR_NULL, "d_flags given without both neighbour flag pointers");
+    if (n_phases == 0) return PGG_OK;
+    const unsigned long long n_span = ((unsigned long long)k_begin + n_phases + 15ull) / 16ull;  // MCS touched
+    if (n_span > PGG_SLAB_MAX_MCS)
+        return fail(PGG_ERR_BAD_PARAM, "the call spans %llu MCS, more than PGG_SLAB_MAX_MCS = %u: split it", n_span, PGG_SLAB_MAX_MCS);
+    if ((unsigned long long)t_begin + n_span > 4294967296ull) return fail(PGG_ERR_BAD_PARAM, "t_begin + MCS spanned exceeds 2^32");
+    if ((unsigned long long)epoch0 + n_phases > 4294967295ull) return fail(PGG_ERR_BAD_PARAM, "epoch0 + n_phases exceeds 2^32 - 1");
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+
+    uint32_t h_table[pgg::kTableSize];
+    rc = pgg_build_accept_table(r, K, h_table);
+    if (rc != PGG_OK) return rc;
+    Scratch tmp(stream);
+    uint64_t* d_seed = nullptr;
+    uint32_t* d_table = nullptr;
+    uint8_t* d_order = nullptr;
+    PGG_CUDA(tmp.alloc((void**)&d_seed, sizeof(uint64_t)));
+    PGG_CUDA(tmp.alloc((void**)&d_table, sizeof(h_table)));
+    PGG_CUDA(tmp.alloc((void**)&d_order, 16 * (size_t)n_span));
+    rc = upload_params(1, &seed, h_table, d_seed, d_table, stream);
+    if (rc != PGG_OK) return rc;
+    pgg::order_kernel<<<((uint32_t)n_span + 127) / 128, 128, 0, stream>>>(d_seed, 1, t_begin, (uint32_t)n_span, (uint32_t)n_span,
+                                                                         order_mode == PGG_ORDER_PERM ? 1 : 0, d_order);
+    PGG_LAUNCHED();
+
+    pgg::SlabArgs a{};
+    a.slab = static_cast<uint8_t*>(d_slab);
+    a.up_halo = static_cast<uint8_t*>(d_up_halo);
+    a.dn_halo = static_cast<uint8_t*>(d_dn_halo);
+    a.seed = d_seed;
+    a.table = d_table;
+    a.order = d_order;
+    a.deltas = reinterpret_cast<unsigned long long*>(d_deltas);
+    a.flags = d_flags;
+    a.up_flag = d_up_flag;
+    a.dn_flag = d_dn_flag;
+    a.L = L;
+    a.row0 = row0;
+    a.n_rows = n_rows;
+    a.t0 = t_begin;
+    const uint32_t n_cls = (n_rows / 4) * (L / 4);
+    const dim3 grid((n_cls + 255) / 256);
+    for (uint32_t p = 0; p < n_phases; ++p) {
+        const uint32_t q = k_begin + p, t = t_begin + (q >> 4), k = q & 15u;
+        if (fmt == PGG_FMT_U8)
+            pgg::phase_slab_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
+        else
+            pgg::phase_slab_kernel<pgg::kFmtBits><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
+        PGG_LAUNCHED();
+    }
+    return PGG_OK;
+}
+
+int32_t pgg_slab_alloc(uint64_t bytes, void** d_out)
+{
+    if (d_out == nullptr) return fail(PGG_ERR_NULL, "d_out is NULL");
+    if (bytes == 0) return fail(PGG_ERR_BAD_PARAM, "bytes is 0");
+    void* p = nullptr;
+    PGG_CUDA(cudaMalloc(&p, bytes));
+    cudaError_t e = cudaMemset(p, 0, bytes);
+    if (e != cudaSuccess) {
+        cudaFree(p);
+        return fail(PGG_ERR_CUDA, "cudaMemset failed: %s", cudaGetErrorString(e));
+    }
+    *d_out = p;
+    return PGG_OK;
+}
+
+int32_t pgg_slab_free(void* d_ptr)
+{
+    if (d_ptr != nullptr) PGG_CUDA(cudaFree(d_ptr));
+    return PGG_OK;
+}
+
+int32_t pgg_slab_ipc_export(void* d_ptr, uint8_t* h_handle64)
+{
+    if (d_ptr == nullptr || h_handle64 == nullptr) return fail(PGG_ERR_NULL, "pointer is NULL");
+    static_assert(sizeof(cudaIpcMemHandle_t) == PGG_SLAB_IPC_HANDLE_BYTES, "IPC handle size");
+    cudaIpcMemHandle_t h;
+    PGG_CUDA(cudaIpcGetMemHandle(&h, d_ptr));
+    std::memcpy(h_handle64, &h, sizeof h);
+    return PGG_OK;
+}
+
+int32_t pgg_slab_ipc_open(const uint8_t* h_handle64, int32_t peer_device, void** d_out)
+{
+    if (h_handle64 == nullptr || d_out == nullptr) return fail(PGG_ERR_NULL, "pointer is NULL");
+    int dev = -1;
+    PGG_CUDA(cudaGetDevice(&dev));
+    if (peer_device >= 0 && peer_device != dev) {
+        int can = 0;
+        PGG_CUDA(cudaDeviceCanAccessPeer(&can, dev, peer_device));
+        if (!can) return fail(PGG_ERR_UNSUPPORTED, "device %d cannot access device %d (no P2P path)", dev, peer_device);
+        cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
+        if (e == cudaErrorPeerAccessAlreadyEnabled) (void)cudaGetLastError();
+        else if (e != cudaSuccess) return fail(PGG_ERR_CUDA, "cudaDeviceEnablePeerAccess(%d) failed: %s", peer_device, cudaGetErrorString(e));
+    }
+    cudaIpcMemHandle_t h;
+    std::memcpy(&h, h_handle64, sizeof h);
+    void* p = nullptr;
+    PGG_CUDA(cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess));
+    *d_out = p;
+    return PGG_OK;
+}
+
+int32_t pgg_slab_ipc_close(void* d_ptr)
+{
+    if (d_ptr != nullptr) PGG_CUDA(cudaIpcCloseMemHandle(d_ptr));
     return PGG_OK;
 }
 

@@ -1,0 +1,154 @@
+// pgg_kernels_slab.cuh -- one phase on a ROW SLAB of a lattice that is sharded over several GPUs
+// ("1-D row slabs, after each phase exchange the 3 boundary rows each way ...
+// fuse the halo push into the phase kernel"; the periodic L x L lattice is PAPER.md:45).
+//
+// A slab is lattice rows [row0, row0 + n_rows) plus three halo rows on either side (the read stencil of
+// an elementary step has radius 3): buffer row q holds lattice row (row0 - 3 + q) mod L,
+// q = 0 .. n_rows + 5, whole rows, in the canonical layout of the lattice (uint8 or bit-packed).
+// Columns stay periodic inside the slab; rows never wrap (the halo rows are the periodic images).
+//
+// The step is V0's (one thread per active site of the slab's own rows, plain global loads) with the site
+// index of the GLOBAL lattice in the Philox counter, so every slab draws exactly what the unsharded sweep
+// draws: the result is bit-identical to pgg_sweep whatever the number of slabs.
+//
+// Halo push, fused.  A site of the slab's first (last) three own rows is also a halo site of the upper
+// (lower) neighbour slab.  The thread that flips it stores the new value into the neighbour's halo copy as
+// well, through `up_halo` / `dn_halo` -- plain device pointers, local or peer (NVLink P2P) memory.  Within
+// a phase nobody reads those copies: a step reads no site of the active class but its own x (same-class
+// sites are >= 4 apart), so the push races with nothing; BETWEEN phases the slabs must be ordered.
+//
+// Ordering between phases, without the host.  flags[1] / flags[2] of a slab count the phases its upper /
+// lower neighbour has completed (written by that neighbour, release at system scope); a phase with global
+// number `epoch` starts when both are >= epoch (so the neighbours' pushes of all earlier phases have
+// landed AND the neighbours have finished reading what this phase is about to overwrite ... one phase of
+// skew at most), and the last CTA to finish posts epoch + 1 to both neighbours.  flags[0] is the CTA
+// counter of that "last one out" detection.  With flags == nullptr the caller orders the phases itself
+// (slabs of one device on one stream: the test path).
+#pragma once
+#include "pgg_common.cuh"
+
+namespace pgg {
+
+struct SlabArgs {
+    uint8_t* slab;               // (n_rows + 6) rows
+    uint8_t* up_halo;            // three rows: the copy of this slab's own rows 0..2 held by the upper neighbour
+    uint8_t* dn_halo;            // three rows: the copy of own rows n_rows-3 .. n_rows-1 held by the lower neighbour
+    const uint64_t* seed;
+    const uint32_t* table;       // 153 thresholds
+    const uint8_t* order;        // [n_mcs spanned][16] phase classes, row 0 = MCS t0
+    unsigned long long* deltas;  // [n_mcs spanned] signed flip sums of this slab's rows, ACCUMULATED; or nullptr
+    unsigned int* flags;         // this slab's three words (see above) or nullptr
+    unsigned int* up_flag;       // the upper neighbour's flags[2] (this slab is its lower neighbour)
+    unsigned int* dn_flag;       // the lower neighbour's flags[1]
+    uint32_t L, row0, n_rows;
+    uint32_t t0;                 // MCS of order[0] / deltas[0]
+};
+
+// Buffer-row accessor with the get(i, j) interface payoff_A / pd_neighbour_count expect: i is a BUFFER row
+// (never wrapped), j a column in [-4, L + 4).
+template <int FMT>
+struct SlabLattice;
+
+template <>
+struct SlabLattice<kFmtU8> {
+    uint8_t* p;
+    int L;
+    __device__ __forceinline__ int get(int q, int j) const { return p[(size_t)q * (size_t)L + (size_t)wrap_coord(j, L)]; }
+    static __device__ __forceinline__ void set(uint8_t* rows, int L, int q, int j, int v)
+    {
+        rows[(size_t)q * (size_t)L + (size_t)j] = (uint8_t)v;
+    }
+};
+
+template <>
+struct SlabLattice<kFmtBits> {
+    uint8_t* p;
+    int L;
+    __device__ __forceinline__ int get(int q, int j) const
+    {
+        const int jj = wrap_coord(j, L);
+        const uint32_t w = reinterpret_cast<const uint32_t*>(p)[(size_t)q * (size_t)(L >> 5) + (size_t)(jj >> 5)];
+        return (int)((w >> (jj & 31)) & 1u);
+    }
+    // eight sites of a class share a word: set / clear the bit atomically (idempotent, unlike a flip)
+    static __device__ __forceinline__ void set(uint8_t* rows, int L, int q, int j, int v)
+    {
+        uint32_t* w = reinterpret_cast<uint32_t*>(rows) + (size_t)q * (size_t)(L >> 5) + (size_t)(j >> 5);
+        if (v) atomicOr(w, 1u << (j & 31)); else atomicAnd(w, ~(1u << (j & 31)));
+    }
+};
+
+template <int FMT>
+__global__ void __launch_bounds__(256)
+phase_slab_kernel(SlabArgs a, uint32_t t, uint32_t k, uint32_t epoch)
+{
+    if (a.flags != nullptr) {
+        if (threadIdx.x == 0) {
+            unsigned int s1, s2, spins = 0;
+            for (;;) {
+                asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(s1) : "l"(a.flags + 1) : "memory");
+                asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(s2) : "l"(a.flags + 2) : "memory");
+                if (s1 >= epoch && s2 >= epoch) break;
+                __nanosleep(200);
+                if (++spins > (1u << 23)) __trap();  // seconds: a lost neighbour must not hang the device
+            }
+        }
+        __syncthreads();
+    }
+    const uint32_t cls = a.order[(size_t)(t - a.t0) * 16 + k];
+    const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
+    const StepKey sk = make_step_key(a.seed[0], t, k, cls);
+    const int L = (int)a.L, m4 = L >> 2, n_rows = (int)a.n_rows;
+    SlabLattice<FMT> lat{a.slab, L};
+    const uint32_t n_cls = (uint32_t)(n_rows >> 2) * (uint32_t)m4;
+    const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+    int delta = 0;
+    if (idx < n_cls) {
+        const int bi = (int)(idx / (uint32_t)m4), bj = (int)(idx - (uint32_t)bi * (uint32_t)m4);
+        const int own = 4 * bi + ci;        // own row of the slab, 0 .. n_rows - 1
+        const int q = own + 3, j = 4 * bj + cj;
+        const uint32_t gi = a.row0 + (uint32_t)own;  // lattice row (row0 + n_rows <= L: never wraps)
+        const int sx = lat.get(q, j);
+        const int s_up = lat.get(q - 1, j), s_dn = lat.get(q + 1, j);
+        const int s_lf = lat.get(q, j - 1), s_rt = lat.get(q, j + 1);
+        if (s_up + s_dn + s_lf + s_rt != 4 * sx) {  // S9
+            uint32_t x0, u;
+            step_draw(sk, gi * (uint32_t)L + (uint32_t)j, x0, u);
+            const int dir = (int)(x0 >> 30);  // 0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1)
+            const int sy = dir == 0 ? s_up : dir == 1 ? s_dn : dir == 2 ? s_lf : s_rt;
+            if (sy != sx) {
+                const int yq = q + (dir == 0 ? -1 : dir == 1 ? 1 : 0);
+                const int yj = j + (dir == 2 ? -1 : dir == 3 ? 1 : 0);
+                const int idx_t = table_index(payoff_A(lat, q, j) - payoff_A(lat, yq, yj), sx - sy);
+                if (u < a.table[idx_t]) {
+                    SlabLattice<FMT>::set(a.slab, L, q, j, sy);
+                    if (own < 3) SlabLattice<FMT>::set(a.up_halo, L, own, j, sy);
+                    if (own >= n_rows - 3) SlabLattice<FMT>::set(a.dn_halo, L, own - (n_rows - 3), j, sy);
+                    delta = sy - sx;
+                }
+            }
+        }
+    }
+    __shared__ int part[8];
+    delta = __reduce_add_sync(0xFFFFFFFFu, delta);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = delta;
+    __syncthreads();  // also: every store of this CTA (own rows, halo pushes) is ordered before thread 0's fence below
+    if (threadIdx.x == 0) {
+        int s = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += part[w];
+        if (s != 0 && a.deltas != nullptr) atomicAdd(a.deltas + (t - a.t0), (unsigned long long)(long long)s);
+        if (a.flags != nullptr) {
+            __threadfence_system();
+            const unsigned int done = atomicAdd(a.flags, 1u);
+            if (done == gridDim.x - 1u) {  // last CTA out: every CTA's stores are visible system-wide
+                atomicExch(a.flags, 0u);
+                __threadfence_system();
+                const unsigned int next = epoch + 1u;
+                asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(a.up_flag), "r"(next) : "memory");
+                asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(a.dn_flag), "r"(next) : "memory");
+            }
+        }
+    }
+}
+
+}  // namespace pgg
