@@ -874,14 +874,16 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     a.row0 = row0;
     a.n_rows = n_rows;
     a.t0 = t_begin;
-    const uint32_t n_cls = (n_rows / 4) * (L / 4);
-    const dim3 grid((n_cls + 255) / 256);
+    // uint8: a thread per active site; bit-packed: a thread per 32-site word of an active row.  8 CTAs of 256
+    // threads per SM at most, grid-stride: the flag protocol costs one wait and one post per CTA.
+    const uint32_t n_items = fmt == PGG_FMT_U8 ? (n_rows / 4) * (L / 4) : (n_rows / 4) * (L / 32);
+    const dim3 grid(std::min<uint32_t>((n_items + 255) / 256, 148u * 8u));
     for (uint32_t p = 0; p < n_phases; ++p) {
         const uint32_t q = k_begin + p, t = t_begin + (q >> 4), k = q & 15u;
         if (fmt == PGG_FMT_U8)
             pgg::phase_slab_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         else
-            pgg::phase_slab_kernel<pgg::kFmtBits><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
+            pgg::phase_slab_words_kernel<<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         PGG_LAUNCHED();
     }
     return PGG_OK;

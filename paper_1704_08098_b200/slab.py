@@ -222,3 +222,57 @@ def run_distributed(full, fmt: int, L: int, r: float, K: float, seed: int, order
         pgg_slab_ipc_close(p)
     sb.free()
     return mine, deltas[:n_mcs]
+
+
+def _time_table(n_mcs: int = 20) -> None:
+    """``python -m paper_1704_08098_b200.slab``: microseconds per phase of the slab kernel on ONE device -- a slab
+    of L / S rows that is its own neighbour (the work and the flag traffic one of S GPUs has; only the timing is
+    meaningful for S > 1) -- beside pgg_sweep on the whole lattice (V0 and AUTO), from the state after 50 MCS."""
+    import torch
+    import paper_1704_08098_b200 as pgg
+
+    def timed(fn, reps=3):
+        best = float("inf")
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        return best * 1e3 / (16 * n_mcs)
+
+    print("| layout | L | pgg_sweep V0 | pgg_sweep AUTO | slab S=1 | S=2 | S=4 | S=8 |")
+    print("|---|---|---|---|---|---|---|---|")
+    for fmt, name in ((FMT_U8, "uint8"), (FMT_BITS, "bits")):
+        for L in (2048, 4096, 16384):
+            shape = (L, L) if fmt == FMT_U8 else (L, L // 32)
+            d = torch.empty(shape, dtype=torch.uint8 if fmt == FMT_U8 else torch.int32, device="cuda")
+            pgg.pgg_init_lattice(d, fmt, L, 0.5, 1)
+            pgg.pgg_sweep(d, fmt, L, 3.8, 0.5, 1, pgg.ORDER_IID, 0, 50)
+            cells = []
+            for variant in (pgg.VARIANT_V0, pgg.VARIANT_AUTO):
+                pgg.pgg_set_variant(variant)
+                c = d.clone()
+                cells.append(timed(lambda: pgg.pgg_sweep(c, fmt, L, 3.8, 0.5, 1, pgg.ORDER_IID, 50, n_mcs)))
+            pgg.pgg_set_variant(pgg.VARIANT_AUTO)
+            for S in (1, 2, 4, 8):
+                n_rows = L // S
+                sb = SlabBuffer(fmt, L, 0, n_rows, d.device)
+                sb.rows().copy_(scatter(d, 0, n_rows))
+                w = wire(sb.ptr, n_rows, sb.ptr, n_rows, sb.ptr, n_rows, fmt, L)
+                epoch = [0]
+
+                def run():
+                    pgg_slab_sweep(sb.ptr, fmt, L, 0, n_rows, 3.8, 0.5, 1, pgg.ORDER_IID, 50, 0, 16 * n_mcs, w["d_up_halo"],
+                                   w["d_dn_halo"], w["d_flags"], w["d_up_flag"], w["d_dn_flag"], epoch[0], None)
+                    epoch[0] += 16 * n_mcs
+
+                cells.append(timed(run))
+                sb.free()
+            print(f"| {name} | {L} | " + " | ".join(f"{x:.1f}" for x in cells) + " |", flush=True)
+
+
+if __name__ == "__main__":
+    _time_table()
