@@ -27,7 +27,6 @@
 #include "pgg_kernels_cluster.cuh"
 #include "pgg_kernels_dtile.cuh"
 #include "pgg_kernels_probe.cuh"
-#include "pgg_kernels_slab.cuh"
 
 namespace {
 
@@ -874,13 +873,34 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     a.row0 = row0;
     a.n_rows = n_rows;
     a.t0 = t_begin;
-    // uint8: a thread per active site; bit-packed: a thread per 32-site word of an active row.  8 CTAs of 256
-    // threads per SM at most, grid-stride: the flag protocol costs one wait and one post per CTA.
+    // Bit-packed slabs of whole LEAN steps (L = 1024 .. 32768, a power of two): LEAN's ring kernel on the slab's buffer.
+    static const bool slab_lean = [] { const char* e = getenv("PGG_SLAB_LEAN"); return e == nullptr || atoi(e) != 0; }();
+    pgg::LeanPlan lplan{};
+    const bool lean = fmt == PGG_FMT_BITS && slab_lean && pgg::lean_plan_slab(L, row0, n_rows, &lplan) == 0;
+    g_variant_used = lean ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;  // pgg_get_variant_used(): which slab kernel ran
+    pgg::PhaseArgs pa{};
+    if (lean) {
+        // the address lattice row 0 would have: buffer row q holds lattice row row0 - 3 + q (rows never wrap in a slab)
+        pa.lats = reinterpret_cast<uint8_t*>(reinterpret_cast<uintptr_t>(d_slab) - ((intptr_t)row0 - 3) * (intptr_t)(L / 8));
+        pa.lat_bytes = 0;
+        pa.seeds = d_seed;
+        pa.tables = d_table;
+        pa.order = d_order;
+        pa.deltas = reinterpret_cast<unsigned long long*>(d_deltas);
+        pa.L = L;
+        pa.order_stride = (uint32_t)n_span;
+        pa.n_mcs = (uint32_t)n_span;
+        pa.t_begin = t_begin;
+    }
+    // General kernels.  uint8: a thread per active site; bit-packed: a thread per 32-site word of an active row.  8 CTAs
+    // of 256 threads per SM at most, grid-stride: the flag protocol costs one wait and one post per CTA.
     const uint32_t n_items = fmt == PGG_FMT_U8 ? (n_rows / 4) * (L / 4) : (n_rows / 4) * (L / 32);
     const dim3 grid(std::min<uint32_t>((n_items + 255) / 256, 148u * 8u));
     for (uint32_t p = 0; p < n_phases; ++p) {
         const uint32_t q = k_begin + p, t = t_begin + (q >> 4), k = q & 15u;
-        if (fmt == PGG_FMT_U8)
+        if (lean)
+            pgg::lean_slab_launch(lplan, pa, t - t_begin, k, a, epoch0 + p, stream);
+        else if (fmt == PGG_FMT_U8)
             pgg::phase_slab_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         else
             pgg::phase_slab_words_kernel<<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);

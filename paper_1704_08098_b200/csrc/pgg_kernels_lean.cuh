@@ -49,6 +49,7 @@
 #pragma once
 #include "pgg_kernels_ring.cuh"
 #include "pgg_stencil_lut.cuh"
+#include "pgg_kernels_slab.cuh"
 
 namespace pgg {
 
@@ -78,8 +79,9 @@ struct LeanPlan {
     uint32_t NS;         // uint8: staging slots
     uint32_t slot_bytes; // uint8: SR * L
     uint32_t nb;         // bands (CTAs) per lattice
-    uint32_t n_steps_total;  // (L / 4) / R
+    uint32_t n_steps_total;  // (L / 4) / R; a row slab: (n_rows / 4) / R
     uint32_t smem_bytes;
+    uint32_t step0;      // a row slab (SLAB): its first step = (row0 / 4) / R; else 0
 };
 
 // 16 lattice bytes (0 / 1 each) -> 16 bits (bit s = byte s) in the low half; the high half is junk.
@@ -139,9 +141,18 @@ __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar)
 // PERSIST: called once per phase from the persistent kernel (no programmatic-dependent-launch fences;
 // the mbarriers are initialised afresh, which is legal because every warp has passed the closing
 // __syncthreads of the previous phase).
-template <int SRC, int GAME, bool PERSIST>
-__device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint32_t k, const LeanPlan& g, bool tables = true)
+// SLAB (bit-packed source only): the "lattice" is a row slab of a lattice sharded over several GPUs
+// (pgg_kernels_slab.cuh).  a.lats is the VIRTUAL base -- the address lattice row 0 would have, so that lattice
+// row i of the slab's buffer (own rows and halo rows) is at a.lats + i * L / 8, i = row0 - 3 .. row0 + n_rows + 2,
+// possibly negative or >= L: rows never wrap, the halo rows are the periodic images.  The steps are those of the
+// whole lattice (g.step0 = the slab's first), so sites and draws are the unsharded sweep's.  A flip in the first /
+// last three own rows is pushed into the neighbour's halo copy; the phase starts when both neighbours have
+// completed `epoch` phases; only the first and the last band wait and post (slab_wait_edge / slab_post_edge).
+template <int SRC, int GAME, bool PERSIST, bool SLAB = false>
+__device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint32_t k, const LeanPlan& g, bool tables = true,
+                                           const SlabArgs* sl = nullptr, uint32_t epoch = 0)
 {
+    static_assert(!SLAB || (SRC == kFmtBits && !PERSIST), "row slabs stream bit rows, one launch per phase");
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int pitch = (int)g.pitch, RC = (int)g.RC;
     const uint32_t NR = g.NR;
@@ -190,12 +201,15 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
     }
     __syncthreads();
     if (!PERSIST) asm volatile("griddepcontrol.wait;" ::: "memory");
+    // the first / last band waits until the upper / lower neighbour slab has completed the previous phase (its pushes
+    // are in my halo rows, its reads of its own halo copy are over); the other bands touch no halo row
+    if (SLAB) slab_wait_edge(*sl, epoch, blockIdx.x == 0, blockIdx.x == gridDim.x - 1);
     const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
     const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
 
     const uint32_t band = blockIdx.x;
-    const uint32_t S0 = (uint32_t)(((unsigned long long)band * g.n_steps_total) / g.nb);
-    const uint32_t S1 = (uint32_t)(((unsigned long long)(band + 1) * g.n_steps_total) / g.nb);
+    const uint32_t S0 = (SLAB ? g.step0 : 0u) + (uint32_t)(((unsigned long long)band * g.n_steps_total) / g.nb);
+    const uint32_t S1 = (SLAB ? g.step0 : 0u) + (uint32_t)(((unsigned long long)(band + 1) * g.n_steps_total) / g.nb);
     const uint32_t n_steps = S1 - S0;
     const uint32_t n_chunks = n_steps ? n_steps + 1 : 0;
     // first lattice row of chunk 0 (the chunk in front of the band's first active row); may be < 0
@@ -206,8 +220,9 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
         // ---------------- producer warp ----------------
         // PERSIST: the flips of the previous phase were made by other SMs through the generic proxy; the
         // grid barrier has ordered them before this point, this fence orders them before the bulk copies
-        if (PERSIST) asm volatile("fence.proxy.async.global;" ::: "memory");
-        int grow = row_c0 < 0 ? row_c0 + (int)L : row_c0;  // lattice row of the current chunk's first row
+        // SLAB: likewise for what the neighbours pushed into my halo rows (ordered before here by the flags)
+        if (PERSIST || SLAB) asm volatile("fence.proxy.async.global;" ::: "memory");
+        int grow = (!SLAB && row_c0 < 0) ? row_c0 + (int)L : row_c0;  // lattice row of the current chunk's first row
         if (SRC == kFmtU8) {
             const uint32_t stage_s = smem_u32(smem_raw + stage_off);
             uint32_t slot = 0, par = 0;  // wait parity of "empty": (use - 1) & 1, use = earlier fills of this slot (>= 1 after the first lap)
@@ -251,23 +266,23 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
                     const bool mirror = slot == NR - 1;  // its last three rows are also staged in front of row 0
                     mbar_expect_tx(bar, (uint32_t)(n + (mirror ? 3 : 0)) * row_bytes_g);
                     int g0 = grow + r0;
-                    if (g0 >= (int)L) g0 -= (int)L;
-                    const int n1st = min(n, (int)L - g0);
+                    if (!SLAB && g0 >= (int)L) g0 -= (int)L;
+                    const int n1st = SLAB ? n : min(n, (int)L - g0);  // (a slab's rows never wrap; g0 may be < 0 or >= L)
                     const uint32_t dst = ring_s + (slot * (uint32_t)RC + (uint32_t)r0) * (uint32_t)pitch;
-                    bulk_g2s(dst, lat + (size_t)g0 * row_bytes_g, (uint32_t)n1st * row_bytes_g, bar);
+                    bulk_g2s(dst, lat + (ptrdiff_t)g0 * (ptrdiff_t)row_bytes_g, (uint32_t)n1st * row_bytes_g, bar);
                     if (n1st < n) bulk_g2s(dst + (uint32_t)n1st * row_bytes_g, lat, (uint32_t)(n - n1st) * row_bytes_g, bar);
                     if (mirror) {
                         int gi = grow + RC - 3;
                         for (int q = 0; q < 3; ++q, ++gi) {  // row by row: the three rows may straddle the lattice end
-                            if (gi >= (int)L) gi -= (int)L;
-                            bulk_g2s(ring_s - (uint32_t)((3 - q) * pitch), lat + (size_t)gi * row_bytes_g, row_bytes_g, bar);
+                            if (!SLAB && gi >= (int)L) gi -= (int)L;
+                            bulk_g2s(ring_s - (uint32_t)((3 - q) * pitch), lat + (ptrdiff_t)gi * (ptrdiff_t)row_bytes_g, row_bytes_g, bar);
                         }
                     }
                 }
                 __syncwarp();
                 if (++slot == NR) { slot = 0; if (first_lap) first_lap = false; else par ^= 1u; }
                 grow += RC;
-                if (grow >= (int)L) grow -= (int)L;
+                if (!SLAB && grow >= (int)L) grow -= (int)L;
             }
         }
     } else if (warp > kLeanConsumers) {
@@ -353,6 +368,11 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
                     lat[w.y] = (uint8_t)(1 - sx);
                 else
                     atomicXor(reinterpret_cast<uint32_t*>(lat) + (w.y >> 5), 1u << (w.y & 31u));
+                if (SLAB) {  // a boundary row of the slab is a halo row of a neighbour: push the new value
+                    const int own = (int)(w.y >> g.lg2L) - (int)sl->row0, n_rows = (int)sl->n_rows, cx = (int)(w.y & (uint32_t)colmask);
+                    if (own < 3) SlabLattice<kFmtBits>::set(sl->up_halo, (int)L, own, cx, 1 - sx);
+                    if (own >= n_rows - 3) SlabLattice<kFmtBits>::set(sl->dn_halo, (int)L, own - (n_rows - 3), cx, 1 - sx);
+                }
                 delta += 1 - 2 * sx;
             }
         };
@@ -493,6 +513,15 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
     __syncthreads();
     if (a.deltas != nullptr && threadIdx.x == 0 && delta_cta != 0)
         atomicAdd(a.deltas + (size_t)b * a.n_mcs + m, (unsigned long long)(long long)delta_cta);
+    // after the __syncthreads: every flip and push of this CTA is issued
+    if (SLAB && threadIdx.x == 0) slab_post_edge(*sl, epoch, blockIdx.x == 0, blockIdx.x == gridDim.x - 1);
+}
+
+// One phase on a bit-packed row slab (pgg_slab_sweep): LEAN's kernel on the slab's buffer.
+__global__ void __launch_bounds__(kLeanThreads, 1)
+phase_lean_slab_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g, SlabArgs sa, uint32_t epoch)
+{
+    lean_phase<kFmtBits, kGamePGG, false, true>(a, m, k, g, true, &sa, epoch);
 }
 
 template <int SRC, int GAME = kGamePGG>
@@ -621,6 +650,7 @@ inline int lean_plan(int fmt, uint32_t L, uint32_t B, LeanPlan* p)
     uint32_t lg = 0;
     while ((1u << lg) < L) ++lg;
     p->lg2L = lg;
+    p->step0 = 0;
     p->pitch = L / 8;
     p->lgWPR = lg - 5;
     const uint32_t wpr = L / 32;
@@ -710,6 +740,42 @@ inline void lean_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t
         cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtU8>, a, m, k, p);
     else
         cudaLaunchKernelEx(&cfg, phase_lean_kernel<kFmtBits>, a, m, k, p);
+}
+
+// LEAN on a row slab: the geometry of the whole lattice (one bit-packed lattice of size L), the steps of the slab.
+// Returns 0, or nonzero if the slab's rows are not whole steps (the caller takes the general slab kernel).
+inline int lean_plan_slab(uint32_t L, uint32_t row0, uint32_t n_rows, LeanPlan* p)
+{
+    if (!lean_supported(kFmtBits, L)) return -1;
+    int rc = lean_plan(kFmtBits, L, 1, p);
+    if (rc != 0) return rc;
+    if ((n_rows / 4) % p->R != 0 || (row0 / 4) % p->R != 0) return -1;
+    cudaError_t e = cudaFuncSetAttribute((const void*)phase_lean_slab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)p->smem_bytes);
+    if (e != cudaSuccess) return (int)e;
+    int dev = 0, sms = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return (int)e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return (int)e;
+    p->n_steps_total = (n_rows / 4) / p->R;
+    p->step0 = (row0 / 4) / p->R;
+    p->nb = p->n_steps_total < (uint32_t)sms ? p->n_steps_total : (uint32_t)sms;
+    return 0;
+}
+
+inline void lean_slab_launch(const LeanPlan& p, const PhaseArgs& a, uint32_t m, uint32_t k, const SlabArgs& sa, uint32_t epoch,
+                             cudaStream_t stream)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(p.nb, 1);
+    cfg.blockDim = dim3(kLeanThreads);
+    cfg.dynamicSmemBytes = p.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel, a, m, k, p, sa, epoch);
 }
 
 // One cooperative launch for MCS [m0, m0 + n_mcs) of B lattices; d_gbar: B zeroed counters.

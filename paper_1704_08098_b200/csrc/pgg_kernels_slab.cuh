@@ -96,30 +96,66 @@ __device__ __forceinline__ void slab_wait(const SlabArgs& a, uint32_t epoch)
     __syncthreads();
 }
 
-// The end of a phase: the CTA's flip count, and -- by the last CTA out -- epoch + 1 to both neighbours.
+// Kernels whose CTAs own contiguous row bands (LEAN on a slab) need less: only the FIRST band reads the top halo
+// and pushes upwards, only the LAST band reads the bottom halo and pushes downwards, and the bands of one slab are
+// ordered among themselves by the launches.  So only those two CTAs wait (each for its own neighbour) and post
+// (each to its own neighbour): no ticket counter, no last-one-out chain; flags[0] is not used.
+__device__ __forceinline__ void slab_wait_edge(const SlabArgs& a, uint32_t epoch, bool top, bool bottom)
+{
+    if (a.flags == nullptr || !(top || bottom)) return;
+    if (threadIdx.x == 0) {
+        unsigned int s1 = epoch, s2 = epoch, spins = 0;
+        for (;;) {
+            if (top) asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(s1) : "l"(a.flags + 1) : "memory");
+            if (bottom) asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(s2) : "l"(a.flags + 2) : "memory");
+            if (s1 >= epoch && s2 >= epoch) break;
+            __nanosleep(200);
+            if (++spins > (1u << 23)) __trap();
+        }
+    }
+    __syncthreads();
+}
+
+// thread 0, after a __syncthreads that follows every store of the CTA
+__device__ __forceinline__ void slab_post_edge(const SlabArgs& a, uint32_t epoch, bool top, bool bottom)
+{
+    if (a.flags == nullptr || !(top || bottom)) return;
+    __threadfence_system();  // fence + relaxed store = release: the band's flips and pushes before its flag
+    const unsigned int next = epoch + 1u;
+    if (top) asm volatile("st.relaxed.sys.global.u32 [%0], %1;" ::"l"(a.up_flag), "r"(next) : "memory");
+    if (bottom) asm volatile("st.relaxed.sys.global.u32 [%0], %1;" ::"l"(a.dn_flag), "r"(next) : "memory");
+}
+
+// The end of a phase, thread 0 of a CTA whose stores are all ordered before this call (after a __syncthreads):
+// its ticket, and -- by the last CTA out -- epoch + 1 to both neighbours.
+__device__ __forceinline__ void slab_post(const SlabArgs& a, uint32_t epoch)
+{
+    if (a.flags == nullptr) return;
+    __threadfence_system();  // this CTA's stores (own rows, pushes into the neighbours) before its ticket
+    const unsigned int done = atomicAdd(a.flags, 1u);
+    if (done == gridDim.x - 1u) {  // last CTA out
+        atomicExch(a.flags, 0u);
+        // fence - ticket ... ticket - fence: every CTA's stores are ordered before what follows, system-wide;
+        // fence + relaxed store = the release of epoch + 1 to the neighbours
+        __threadfence_system();
+        const unsigned int next = epoch + 1u;
+        asm volatile("st.relaxed.sys.global.u32 [%0], %1;" ::"l"(a.up_flag), "r"(next) : "memory");
+        asm volatile("st.relaxed.sys.global.u32 [%0], %1;" ::"l"(a.dn_flag), "r"(next) : "memory");
+    }
+}
+
+// The end of a phase for the kernels of this file: the CTA's flip count, then slab_post.
 __device__ __forceinline__ void slab_finish(const SlabArgs& a, int delta, uint32_t t, uint32_t epoch)
 {
     __shared__ int part[8];
     delta = __reduce_add_sync(0xFFFFFFFFu, delta);
     if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = delta;
-    __syncthreads();  // also: every store of this CTA (own rows, halo pushes) is ordered before thread 0's fence below
+    __syncthreads();  // also: every store of this CTA (own rows, halo pushes) is ordered before thread 0's fence
     if (threadIdx.x == 0) {
         int s = 0;
         for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += part[w];
         if (s != 0 && a.deltas != nullptr) atomicAdd(a.deltas + (t - a.t0), (unsigned long long)(long long)s);
-        if (a.flags != nullptr) {
-            __threadfence_system();  // this CTA's stores (own rows, pushes into the neighbours) before its ticket
-            const unsigned int done = atomicAdd(a.flags, 1u);
-            if (done == gridDim.x - 1u) {  // last CTA out
-                atomicExch(a.flags, 0u);
-                // fence - ticket ... ticket - fence: every CTA's stores are ordered before what follows, system-wide;
-                // fence + relaxed store = the release of epoch + 1 to the neighbours
-                __threadfence_system();
-                const unsigned int next = epoch + 1u;
-                asm volatile("st.relaxed.sys.global.u32 [%0], %1;" ::"l"(a.up_flag), "r"(next) : "memory");
-                asm volatile("st.relaxed.sys.global.u32 [%0], %1;" ::"l"(a.dn_flag), "r"(next) : "memory");
-            }
-        }
+        slab_post(a, epoch);
     }
 }
 

@@ -111,6 +111,34 @@ def test_slabs_equal_pgg_sweep_on_a_larger_lattice(fmt):
     assert np.array_equal(got, ref) and np.array_equal(counts, ref_counts)
 
 
+@pytest.mark.parametrize("L,S", [(1024, 1), (1024, 2), (1024, 4), (1024, 16), (2048, 8), (4096, 4)])
+def test_lean_slabs_equal_the_unsharded_oracle(L, S):
+    """Bit-packed slabs of whole LEAN steps run LEAN's ring kernel on the slab's buffer (rows never wrap, the virtual
+    lattice base, the steps of the whole lattice, the push from the level-2 write): same bar, against the oracle."""
+    n_mcs, seed, r = 3, 31, 3.8
+    lat0 = wl.random_lattice(L, 0.5, 17)
+    ref = lat0.copy()
+    ref_counts, _ = orc.sweep(ref, r, K, seed, orc.ORDER_IID, 7, n_mcs, n_threads=orc.max_threads())
+    got, counts, flags = run_slabs(lat0, pgg.FMT_BITS, S, r, seed, pgg.ORDER_IID, 7, n_mcs, use_flags=True)
+    assert pgg.pgg_get_variant_used() == pgg.VARIANT_LEAN
+    assert np.array_equal(got, ref), f"{int((got != ref).sum())} sites differ"
+    assert np.array_equal(counts, ref_counts)
+    assert flags == [[0, 16 * n_mcs, 16 * n_mcs]] * S
+
+
+def test_lean_slab_structured_state_and_ragged_split_falls_back():
+    """Blobs and stripes (long quiet stretches, busy boundaries) on LEAN slabs; a split into slabs that are not whole
+    LEAN steps (3 slabs of L = 1024: 344, 340, 340 rows) takes the general word kernel and gives the same lattice."""
+    L, n_mcs, seed, r = 1024, 2, 5, 4.4
+    for lat0 in (wl.blobs_lattice(L, 9), wl.stripes_lattice(L, 5)):
+        ref = lat0.copy()
+        ref_counts, _ = orc.sweep(ref, r, K, seed, orc.ORDER_PERM, 0, n_mcs, n_threads=orc.max_threads())
+        for S, want in ((4, pgg.VARIANT_LEAN), (3, pgg.VARIANT_V0)):
+            got, counts, _ = run_slabs(lat0, pgg.FMT_BITS, S, r, seed, pgg.ORDER_PERM, 0, n_mcs, use_flags=True)
+            assert pgg.pgg_get_variant_used() == want
+            assert np.array_equal(got, ref) and np.array_equal(counts, ref_counts)
+
+
 def test_one_call_for_many_phases_on_a_single_slab():
     """A single slab is its own neighbour both ways, so ONE call may run all phases of several MCS (the way
     run_distributed calls it): mid-MCS start, flags on, against the oracle."""
