@@ -269,6 +269,9 @@ int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, d
 #define PGG_SLAB_MAX_MCS 4096u
 #define PGG_SLAB_IPC_HANDLE_BYTES 64
 uint64_t pgg_slab_bytes(int32_t fmt, uint32_t L, uint32_t n_rows);
+/* Row granularity of the fast slab kernel: a slab whose row0 and n_rows are multiples of it runs LEAN's ring kernel
+ * (bit-packed, L = 1024 .. 32768 a power of two: 4 R rows), else 4.  Uses the current CUDA device; 4 on any failure. */
+uint32_t pgg_slab_step_rows(int32_t fmt, uint32_t L);
 int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
                        uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
                        void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,

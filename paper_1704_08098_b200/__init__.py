@@ -44,6 +44,7 @@ SIGNATURES = {
     "pgg_pd_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32] + [C.c_double] * 5 +
                      [C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p]),
     "pgg_slab_bytes": (C.c_uint64, [C.c_int32, C.c_uint32, C.c_uint32]),
+    "pgg_slab_step_rows": (C.c_uint32, [C.c_int32, C.c_uint32]),
     "pgg_slab_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_double, C.c_double,
                                    C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p,
                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]),
@@ -164,6 +165,11 @@ SLAB_IPC_HANDLE_BYTES = 64
 
 def pgg_slab_bytes(fmt: int, L: int, n_rows: int) -> int:
     return int(lib().pgg_slab_bytes(fmt, L, n_rows))
+
+
+def pgg_slab_step_rows(fmt: int, L: int) -> int:
+    """Row granularity (row0, n_rows) at which a slab runs the fast kernel; needs a CUDA device."""
+    return int(lib().pgg_slab_step_rows(fmt, L))
 
 
 def pgg_slab_sweep(d_slab, fmt: int, L: int, row0: int, n_rows: int, r: float, K: float, seed: int, order_mode: int,

@@ -813,6 +813,13 @@ uint64_t pgg_slab_bytes(int32_t fmt, uint32_t L, uint32_t n_rows)
     return row * ((unsigned long long)n_rows + 6ull);
 }
 
+uint32_t pgg_slab_step_rows(int32_t fmt, uint32_t L)
+{
+    pgg::LeanPlan p{};
+    if (fmt != PGG_FMT_BITS || !pgg::lean_supported(fmt, L) || pgg::lean_plan(fmt, L, 1, &p) != 0) return 4;
+    return 4 * p.R;
+}
+
 int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
                        uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
                        void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,

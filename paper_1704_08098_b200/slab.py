@@ -16,20 +16,24 @@ driver; its wiring is covered on CPU with gloo (tests/test_slab_host.py).
 from __future__ import annotations
 
 from . import (FMT_BITS, FMT_U8, SLAB_MAX_MCS, pgg_slab_alloc, pgg_slab_bytes, pgg_slab_free, pgg_slab_ipc_close,
-               pgg_slab_ipc_export, pgg_slab_ipc_open, pgg_slab_sweep)
+               pgg_slab_ipc_export, pgg_slab_ipc_open, pgg_slab_step_rows, pgg_slab_sweep)
 
 HALO = 3          # rows: the read stencil of an elementary step has radius 3
 FLAG_BYTES = 256  # the three flag words of a slab, in a block of their own behind the rows
 
 
-def slab_rows(L: int, world: int, rank: int) -> tuple[int, int]:
-    """-> (row0, n_rows) of rank's slab: the L/4 row groups split as evenly as possible, in rank order."""
-    groups = L // 4
+def slab_rows(L: int, world: int, rank: int, align: int = 4) -> tuple[int, int]:
+    """-> (row0, n_rows) of rank's slab: the L/align row groups split as evenly as possible, in rank order.
+    align = 4 (a class row every four rows) or a multiple the fast kernel wants (pgg_slab_step_rows); an align
+    the lattice is too small for (fewer groups than ranks) falls back to 4."""
+    if align % 4 or align < 4 or L % align or L // align < world:
+        align = 4
+    groups = L // align
     if L % 4 or not 1 <= world <= groups or not 0 <= rank < world:
         raise ValueError(f"L = {L}, world = {world}, rank = {rank}: need L % 4 == 0 and 1 <= world <= L / 4")
     base, rem = divmod(groups, world)
     g0 = rank * base + min(rank, rem)
-    return 4 * g0, 4 * (base + (1 if rank < rem else 0))
+    return align * g0, align * (base + (1 if rank < rem else 0))
 
 
 def neighbours(world: int, rank: int) -> tuple[int, int]:
@@ -129,11 +133,12 @@ class LocalSlabs:
     runs phase p before any runs p + 1), with or without the flag protocol; the result equals pgg_sweep on the
     whole lattice bit for bit."""
 
-    def __init__(self, full, fmt: int, L: int, n_slabs: int, use_flags: bool = True):
+    def __init__(self, full, fmt: int, L: int, n_slabs: int, use_flags: bool = True, align: int | None = None):
         self.fmt, self.L, self.S, self.use_flags = fmt, L, n_slabs, use_flags
+        self.align = pgg_slab_step_rows(fmt, L) if align is None else align  # None: what the fast kernel wants
         self.slabs = []
         for rank in range(n_slabs):
-            row0, n_rows = slab_rows(L, n_slabs, rank)
+            row0, n_rows = slab_rows(L, n_slabs, rank, self.align)
             sb = SlabBuffer(fmt, L, row0, n_rows, full.device)
             sb.rows().copy_(scatter(full, row0, n_rows))
             self.slabs.append(sb)
@@ -191,7 +196,7 @@ def run_distributed(full, fmt: int, L: int, r: float, K: float, seed: int, order
     import torch
     import torch.distributed as dist
     world, rank = dist.get_world_size(group), dist.get_rank(group)
-    row0, n_rows = slab_rows(L, world, rank)
+    row0, n_rows = slab_rows(L, world, rank, pgg_slab_step_rows(fmt, L))  # the same on every rank
     sb = SlabBuffer(fmt, L, row0, n_rows, full.device)
     sb.rows().copy_(scatter(full, row0, n_rows))
     torch.cuda.synchronize()

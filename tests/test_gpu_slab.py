@@ -54,9 +54,9 @@ def to_host(d_lat, fmt, L):
     return bits.reshape(words.shape[:-1] + (L,)).astype(np.uint8)
 
 
-def run_slabs(lat0, fmt, S, r, seed, order, t_begin, n_mcs, use_flags):
+def run_slabs(lat0, fmt, S, r, seed, order, t_begin, n_mcs, use_flags, align=None):
     L = lat0.shape[0]
-    ls = slab.LocalSlabs(to_device(lat0, fmt), fmt, L, S, use_flags=use_flags)
+    ls = slab.LocalSlabs(to_device(lat0, fmt), fmt, L, S, use_flags=use_flags, align=align)
     try:
         deltas = ls.sweep(r, K, seed, order, t_begin, n_mcs)
         torch.cuda.synchronize()
@@ -111,7 +111,7 @@ def test_slabs_equal_pgg_sweep_on_a_larger_lattice(fmt):
     assert np.array_equal(got, ref) and np.array_equal(counts, ref_counts)
 
 
-@pytest.mark.parametrize("L,S", [(1024, 1), (1024, 2), (1024, 4), (1024, 16), (2048, 8), (4096, 4)])
+@pytest.mark.parametrize("L,S", [(1024, 1), (1024, 2), (1024, 3), (1024, 4), (1024, 16), (2048, 8), (4096, 4)])
 def test_lean_slabs_equal_the_unsharded_oracle(L, S):
     """Bit-packed slabs of whole LEAN steps run LEAN's ring kernel on the slab's buffer (rows never wrap, the virtual
     lattice base, the steps of the whole lattice, the push from the level-2 write): same bar, against the oracle."""
@@ -128,13 +128,14 @@ def test_lean_slabs_equal_the_unsharded_oracle(L, S):
 
 def test_lean_slab_structured_state_and_ragged_split_falls_back():
     """Blobs and stripes (long quiet stretches, busy boundaries) on LEAN slabs; a split into slabs that are not whole
-    LEAN steps (3 slabs of L = 1024: 344, 340, 340 rows) takes the general word kernel and gives the same lattice."""
+    LEAN steps (align = 4; 3 slabs of L = 1024: 344, 340, 340 rows) takes the general word kernel and gives the same
+    lattice.  (By default the split follows pgg_slab_step_rows: 384, 320, 320 rows, all on LEAN.)"""
     L, n_mcs, seed, r = 1024, 2, 5, 4.4
     for lat0 in (wl.blobs_lattice(L, 9), wl.stripes_lattice(L, 5)):
         ref = lat0.copy()
         ref_counts, _ = orc.sweep(ref, r, K, seed, orc.ORDER_PERM, 0, n_mcs, n_threads=orc.max_threads())
-        for S, want in ((4, pgg.VARIANT_LEAN), (3, pgg.VARIANT_V0)):
-            got, counts, _ = run_slabs(lat0, pgg.FMT_BITS, S, r, seed, pgg.ORDER_PERM, 0, n_mcs, use_flags=True)
+        for S, align, want in ((4, None, pgg.VARIANT_LEAN), (3, 4, pgg.VARIANT_V0)):
+            got, counts, _ = run_slabs(lat0, pgg.FMT_BITS, S, r, seed, pgg.ORDER_PERM, 0, n_mcs, use_flags=True, align=align)
             assert pgg.pgg_get_variant_used() == want
             assert np.array_equal(got, ref) and np.array_equal(counts, ref_counts)
 

@@ -24,6 +24,16 @@ def test_slab_rows_partition_the_lattice(L, world):
         slab.slab_rows(L, L // 4 + 1, 0)
 
 
+def test_slab_rows_with_the_fast_kernels_alignment():
+    """align = 4 R rows (pgg_slab_step_rows): every slab a whole number of LEAN steps; too few groups -> align 4."""
+    rows = [slab.slab_rows(1024, 3, q, 64) for q in range(3)]
+    assert rows == [(0, 384), (384, 320), (704, 320)]
+    rows = [slab.slab_rows(16384, 3, q, 8) for q in range(3)]
+    assert sum(n for _, n in rows) == 16384 and all(r0 % 8 == 0 and n % 8 == 0 for r0, n in rows)
+    assert [slab.slab_rows(1024, 32, q, 64)[1] for q in range(32)] == [32] * 32       # 16 groups < 32 ranks: align 4
+    assert slab.slab_rows(96, 5, 0, 64) == slab.slab_rows(96, 5, 0)                    # L % align != 0: align 4
+
+
 def test_scatter_has_periodic_halos_and_gather_inverts():
     L, world = 32, 3
     full = torch.arange(L * L, dtype=torch.int64).reshape(L, L)
