@@ -253,11 +253,11 @@ int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, d
  *               (ceil((k_begin + n_phases) / 16)): the signed number of flips of this slab's own rows in MCS
  *               t_begin + m is ADDED to d_deltas[m].  The rho_C trace (Eq. 4) is the initial count
  *               plus the running sum of the deltas summed over all slabs (one all-reduce per call, not per phase).
- * At most PGG_SLAB_MAX_MCS MCS per call.  Kernels: a bit-packed slab of whole LEAN steps (L = 1024 .. 32768, a power
- * of two; row0 and n_rows multiples of 4R, R = max(1, 16384 / L) active rows per step, doubled from L = 16384) runs
- * LEAN's ring kernel on the slab's buffer, and only its first / last row band waits for and posts to the upper /
- * lower neighbour; any other slab runs a general kernel (uint8: a thread per active site; bits: a thread per 32-site
- * word) in which every CTA waits and the last CTA out posts.  pgg_get_variant_used() says which
+ * At most PGG_SLAB_MAX_MCS MCS per call.  Kernels: a slab of whole LEAN steps (L = 1024 .. 32768, a power of two;
+ * row0 and n_rows multiples of pgg_slab_step_rows(fmt, L)) runs LEAN's ring kernel on the slab's buffer, and only
+ * its first / last row band waits for and posts to the upper / lower neighbour; any other slab runs a general
+ * kernel (uint8: a thread per active site; bits: a thread per 32-site word) in which every CTA waits and the
+ * last CTA out posts.  pgg_get_variant_used() says which
  * (PGG_VARIANT_LEAN / PGG_VARIANT_V0); the environment variable PGG_SLAB_LEAN=0 forces the general kernel.
  * Errors: PGG_ERR_NULL, PGG_ERR_BAD_L, PGG_ERR_ALIGN, PGG_ERR_BAD_PARAM (rows, k_begin, r, K, span, epochs),
  * PGG_ERR_UNSUPPORTED (fmt, order_mode), PGG_ERR_CUDA.  n_phases == 0 is a no-op.
@@ -270,7 +270,8 @@ int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, d
 #define PGG_SLAB_IPC_HANDLE_BYTES 64
 uint64_t pgg_slab_bytes(int32_t fmt, uint32_t L, uint32_t n_rows);
 /* Row granularity of the fast slab kernel: a slab whose row0 and n_rows are multiples of it runs LEAN's ring kernel
- * (bit-packed, L = 1024 .. 32768 a power of two: 4 R rows), else 4.  Uses the current CUDA device; 4 on any failure. */
+ * (L = 1024 .. 32768, a power of two: 4 R rows, R = LEAN's active rows per step for this layout), else 4.  Uses the
+ * current CUDA device; 4 on any failure.                                                                          */
 uint32_t pgg_slab_step_rows(int32_t fmt, uint32_t L);
 int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
                        uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,

@@ -816,7 +816,7 @@ uint64_t pgg_slab_bytes(int32_t fmt, uint32_t L, uint32_t n_rows)
 uint32_t pgg_slab_step_rows(int32_t fmt, uint32_t L)
 {
     pgg::LeanPlan p{};
-    if (fmt != PGG_FMT_BITS || !pgg::lean_supported(fmt, L) || pgg::lean_plan(fmt, L, 1, &p) != 0) return 4;
+    if ((fmt != PGG_FMT_BITS && fmt != PGG_FMT_U8) || !pgg::lean_supported(fmt, L) || pgg::lean_plan(fmt, L, 1, &p) != 0) return 4;
     return 4 * p.R;
 }
 
@@ -880,15 +880,15 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     a.row0 = row0;
     a.n_rows = n_rows;
     a.t0 = t_begin;
-    // Bit-packed slabs of whole LEAN steps (L = 1024 .. 32768, a power of two): LEAN's ring kernel on the slab's buffer.
+    // Slabs of whole LEAN steps (L = 1024 .. 32768, a power of two): LEAN's ring kernel on the slab's buffer.
     static const bool slab_lean = [] { const char* e = getenv("PGG_SLAB_LEAN"); return e == nullptr || atoi(e) != 0; }();
     pgg::LeanPlan lplan{};
-    const bool lean = fmt == PGG_FMT_BITS && slab_lean && pgg::lean_plan_slab(L, row0, n_rows, &lplan) == 0;
+    const bool lean = slab_lean && pgg::lean_plan_slab(fmt, L, row0, n_rows, &lplan) == 0;
     g_variant_used = lean ? PGG_VARIANT_LEAN : PGG_VARIANT_V0;  // pgg_get_variant_used(): which slab kernel ran
     pgg::PhaseArgs pa{};
     if (lean) {
         // the address lattice row 0 would have: buffer row q holds lattice row row0 - 3 + q (rows never wrap in a slab)
-        pa.lats = reinterpret_cast<uint8_t*>(reinterpret_cast<uintptr_t>(d_slab) - ((intptr_t)row0 - 3) * (intptr_t)(L / 8));
+        pa.lats = reinterpret_cast<uint8_t*>(reinterpret_cast<uintptr_t>(d_slab) - ((intptr_t)row0 - 3) * (intptr_t)(fmt == PGG_FMT_U8 ? L : L / 8));
         pa.lat_bytes = 0;
         pa.seeds = d_seed;
         pa.tables = d_table;
@@ -906,7 +906,7 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     for (uint32_t p = 0; p < n_phases; ++p) {
         const uint32_t q = k_begin + p, t = t_begin + (q >> 4), k = q & 15u;
         if (lean)
-            pgg::lean_slab_launch(lplan, pa, t - t_begin, k, a, epoch0 + p, stream);
+            pgg::lean_slab_launch(lplan, fmt, pa, t - t_begin, k, a, epoch0 + p, stream);
         else if (fmt == PGG_FMT_U8)
             pgg::phase_slab_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         else

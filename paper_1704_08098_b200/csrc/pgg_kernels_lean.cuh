@@ -141,9 +141,9 @@ __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar)
 // PERSIST: called once per phase from the persistent kernel (no programmatic-dependent-launch fences;
 // the mbarriers are initialised afresh, which is legal because every warp has passed the closing
 // __syncthreads of the previous phase).
-// SLAB (bit-packed source only): the "lattice" is a row slab of a lattice sharded over several GPUs
+// SLAB: the "lattice" is a row slab of a lattice sharded over several GPUs
 // (pgg_kernels_slab.cuh).  a.lats is the VIRTUAL base -- the address lattice row 0 would have, so that lattice
-// row i of the slab's buffer (own rows and halo rows) is at a.lats + i * L / 8, i = row0 - 3 .. row0 + n_rows + 2,
+// row i of the slab's buffer (own rows and halo rows) is at a.lats + i * (bytes per row), i = row0 - 3 .. row0 + n_rows + 2,
 // possibly negative or >= L: rows never wrap, the halo rows are the periodic images.  The steps are those of the
 // whole lattice (g.step0 = the slab's first), so sites and draws are the unsharded sweep's.  A flip in the first /
 // last three own rows is pushed into the neighbour's halo copy; the phase starts when both neighbours have
@@ -152,7 +152,7 @@ template <int SRC, int GAME, bool PERSIST, bool SLAB = false>
 __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint32_t k, const LeanPlan& g, bool tables = true,
                                            const SlabArgs* sl = nullptr, uint32_t epoch = 0)
 {
-    static_assert(!SLAB || (SRC == kFmtBits && !PERSIST), "row slabs stream bit rows, one launch per phase");
+    static_assert(!SLAB || !PERSIST, "row slabs: one launch per phase");
     extern __shared__ __align__(128) uint8_t smem_raw[];
     const int pitch = (int)g.pitch, RC = (int)g.RC;
     const uint32_t NR = g.NR;
@@ -241,17 +241,17 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
                         const int n = r1 - r0;
                         mbar_expect_tx(bar, (uint32_t)n * L);
                         int g0 = grow + r0;
-                        if (g0 >= (int)L) g0 -= (int)L;
-                        const int n1st = min(n, (int)L - g0);
+                        if (!SLAB && g0 >= (int)L) g0 -= (int)L;
+                        const int n1st = SLAB ? n : min(n, (int)L - g0);
                         const uint32_t dst = stage_s + slot * g.slot_bytes + (uint32_t)(r0 - (int)(j * g.SR)) * L;
-                        bulk_g2s(dst, lat + (size_t)g0 * L, (uint32_t)n1st * L, bar);
+                        bulk_g2s(dst, lat + (ptrdiff_t)g0 * (ptrdiff_t)L, (uint32_t)n1st * L, bar);
                         if (n1st < n) bulk_g2s(dst + (uint32_t)n1st * L, lat, (uint32_t)(n - n1st) * L, bar);
                     }
                     __syncwarp();
                     if (++slot == g.NS) { slot = 0; if (first_lap) first_lap = false; else par ^= 1u; }
                 }
                 grow += RC;
-                if (grow >= (int)L) grow -= (int)L;
+                if (!SLAB && grow >= (int)L) grow -= (int)L;
             }
         } else {
             const uint32_t ring_s = smem_u32(ring0);
@@ -370,8 +370,8 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
                     atomicXor(reinterpret_cast<uint32_t*>(lat) + (w.y >> 5), 1u << (w.y & 31u));
                 if (SLAB) {  // a boundary row of the slab is a halo row of a neighbour: push the new value
                     const int own = (int)(w.y >> g.lg2L) - (int)sl->row0, n_rows = (int)sl->n_rows, cx = (int)(w.y & (uint32_t)colmask);
-                    if (own < 3) SlabLattice<kFmtBits>::set(sl->up_halo, (int)L, own, cx, 1 - sx);
-                    if (own >= n_rows - 3) SlabLattice<kFmtBits>::set(sl->dn_halo, (int)L, own - (n_rows - 3), cx, 1 - sx);
+                    if (own < 3) SlabLattice<SRC>::set(sl->up_halo, (int)L, own, cx, 1 - sx);
+                    if (own >= n_rows - 3) SlabLattice<SRC>::set(sl->dn_halo, (int)L, own - (n_rows - 3), cx, 1 - sx);
                 }
                 delta += 1 - 2 * sx;
             }
@@ -517,11 +517,12 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
     if (SLAB && threadIdx.x == 0) slab_post_edge(*sl, epoch, blockIdx.x == 0, blockIdx.x == gridDim.x - 1);
 }
 
-// One phase on a bit-packed row slab (pgg_slab_sweep): LEAN's kernel on the slab's buffer.
-__global__ void __launch_bounds__(kLeanThreads, 1)
+// One phase on a row slab (pgg_slab_sweep): LEAN's kernel on the slab's buffer, rows of layout SRC.
+template <int SRC>
+__global__ void __launch_bounds__(SRC == kFmtU8 ? kLeanThreadsU8 : kLeanThreads, 1)
 phase_lean_slab_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g, SlabArgs sa, uint32_t epoch)
 {
-    lean_phase<kFmtBits, kGamePGG, false, true>(a, m, k, g, true, &sa, epoch);
+    lean_phase<SRC, kGamePGG, false, true>(a, m, k, g, true, &sa, epoch);
 }
 
 template <int SRC, int GAME = kGamePGG>
@@ -744,14 +745,14 @@ inline void lean_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t
 
 // LEAN on a row slab: the geometry of the whole lattice (one bit-packed lattice of size L), the steps of the slab.
 // Returns 0, or nonzero if the slab's rows are not whole steps (the caller takes the general slab kernel).
-inline int lean_plan_slab(uint32_t L, uint32_t row0, uint32_t n_rows, LeanPlan* p)
+inline int lean_plan_slab(int fmt, uint32_t L, uint32_t row0, uint32_t n_rows, LeanPlan* p)
 {
-    if (!lean_supported(kFmtBits, L)) return -1;
-    int rc = lean_plan(kFmtBits, L, 1, p);
+    if (!lean_supported(fmt, L)) return -1;
+    int rc = lean_plan(fmt, L, 1, p);
     if (rc != 0) return rc;
     if ((n_rows / 4) % p->R != 0 || (row0 / 4) % p->R != 0) return -1;
-    cudaError_t e = cudaFuncSetAttribute((const void*)phase_lean_slab_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)p->smem_bytes);
+    const void* fn = fmt == kFmtU8 ? (const void*)phase_lean_slab_kernel<kFmtU8> : (const void*)phase_lean_slab_kernel<kFmtBits>;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes);
     if (e != cudaSuccess) return (int)e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return (int)e;
@@ -762,12 +763,12 @@ inline int lean_plan_slab(uint32_t L, uint32_t row0, uint32_t n_rows, LeanPlan* 
     return 0;
 }
 
-inline void lean_slab_launch(const LeanPlan& p, const PhaseArgs& a, uint32_t m, uint32_t k, const SlabArgs& sa, uint32_t epoch,
-                             cudaStream_t stream)
+inline void lean_slab_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t m, uint32_t k, const SlabArgs& sa,
+                             uint32_t epoch, cudaStream_t stream)
 {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p.nb, 1);
-    cfg.blockDim = dim3(kLeanThreads);
+    cfg.blockDim = dim3(fmt == kFmtU8 ? kLeanThreadsU8 : kLeanThreads);
     cfg.dynamicSmemBytes = p.smem_bytes;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
@@ -775,7 +776,10 @@ inline void lean_slab_launch(const LeanPlan& p, const PhaseArgs& a, uint32_t m, 
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel, a, m, k, p, sa, epoch);
+    if (fmt == kFmtU8)
+        cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel<kFmtU8>, a, m, k, p, sa, epoch);
+    else
+        cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel<kFmtBits>, a, m, k, p, sa, epoch);
 }
 
 // One cooperative launch for MCS [m0, m0 + n_mcs) of B lattices; d_gbar: B zeroed counters.

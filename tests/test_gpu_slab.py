@@ -111,15 +111,17 @@ def test_slabs_equal_pgg_sweep_on_a_larger_lattice(fmt):
     assert np.array_equal(got, ref) and np.array_equal(counts, ref_counts)
 
 
+@pytest.mark.parametrize("fmt", FMTS)
 @pytest.mark.parametrize("L,S", [(1024, 1), (1024, 2), (1024, 3), (1024, 4), (1024, 16), (2048, 8), (4096, 4)])
-def test_lean_slabs_equal_the_unsharded_oracle(L, S):
-    """Bit-packed slabs of whole LEAN steps run LEAN's ring kernel on the slab's buffer (rows never wrap, the virtual
-    lattice base, the steps of the whole lattice, the push from the level-2 write): same bar, against the oracle."""
+def test_lean_slabs_equal_the_unsharded_oracle(fmt, L, S):
+    """Slabs of whole LEAN steps run LEAN's ring kernel on the slab's buffer (rows never wrap, the virtual lattice
+    base, the steps of the whole lattice, the push from the level-2 write; uint8 rows are packed to bits on arrival
+    as in the unsharded kernel): same bar, against the oracle."""
     n_mcs, seed, r = 3, 31, 3.8
     lat0 = wl.random_lattice(L, 0.5, 17)
     ref = lat0.copy()
     ref_counts, _ = orc.sweep(ref, r, K, seed, orc.ORDER_IID, 7, n_mcs, n_threads=orc.max_threads())
-    got, counts, flags = run_slabs(lat0, pgg.FMT_BITS, S, r, seed, pgg.ORDER_IID, 7, n_mcs, use_flags=True)
+    got, counts, flags = run_slabs(lat0, fmt, S, r, seed, pgg.ORDER_IID, 7, n_mcs, use_flags=True)
     assert pgg.pgg_get_variant_used() == pgg.VARIANT_LEAN
     assert np.array_equal(got, ref), f"{int((got != ref).sum())} sites differ"
     assert np.array_equal(counts, ref_counts)
