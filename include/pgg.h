@@ -248,7 +248,11 @@ int32_t pgg_pd_sweep(void* d_lat, int32_t fmt, uint32_t L, double R, double S, d
  *               system scope; a wait of seconds traps instead of hanging) and, complete, stores e + 1 to both
  *               neighbours (release, system scope).  All slabs of the lattice must run the same phases with the
  *               same epoch numbers; epoch0 continues from call to call.  No host synchronisation, no NCCL on
- *               the data path: neighbouring slabs are at most one phase apart.
+ *               the data path: neighbouring slabs are at most one phase apart.  ONE SLAB PER DEVICE when the flags
+ *               are meant to wait: a waiting kernel holds its SMs, so two slabs of one device on different streams
+ *               can starve each other until the wait traps.  Slabs that share a device are launched phase by phase
+ *               in dependency order on one stream (every slab runs phase p before any runs p + 1); the flags are
+ *               then always found set (paper_1704_08098_b200/slab.py: LocalSlabs).
  *   d_deltas : NULL or device array of uint64 (two's complement), one per MCS the call touches
  *               (ceil((k_begin + n_phases) / 16)): the signed number of flips of this slab's own rows in MCS
  *               t_begin + m is ADDED to d_deltas[m].  The rho_C trace (Eq. 4) is the initial count
