@@ -279,5 +279,79 @@ def _time_table(n_mcs: int = 20) -> None:
             print(f"| {name} | {L} | " + " | ".join(f"{x:.1f}" for x in cells) + " |", flush=True)
 
 
+def _run_sharded(args) -> None:
+    """One process per GPU (torchrun): ONE lattice of size L in row slabs, ``--mcs`` MCS from a Bernoulli(0.5) start;
+    rank 0 prints one JSON line (updates/s of the whole lattice, device time as the max over ranks).  ``--check``
+    also runs the unsharded pgg_sweep on every rank and compares its rows and the count trace with the slabs'."""
+    import json
+    import os
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1704_08098_b200 as pgg
+
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", 0)))
+    if not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl" if world > 1 else "gloo", rank=rank, world_size=world)
+    fmt = FMT_BITS if args.fmt == "bits" else FMT_U8
+    L, n, r, K, seed = args.L, args.mcs, args.r, 0.5, args.seed
+    full = torch.empty((L, L) if fmt == FMT_U8 else (L, L // 32), dtype=torch.uint8 if fmt == FMT_U8 else torch.int32,
+                       device="cuda")
+    pgg.pgg_init_lattice(full, fmt, L, 0.5, seed)   # every rank makes the same seeded start; it keeps only its slab
+    count0 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    pgg.pgg_density(full, fmt, L, count0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    dist.barrier()
+    e0.record()
+    mine, deltas = run_distributed(full, fmt, L, r, K, seed, pgg.ORDER_IID, 0, n)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda" if world > 1 else "cpu")
+    dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    counts = count0 + torch.cumsum(deltas, 0)
+    ok = None
+    if args.check:
+        cnt = torch.zeros(n, dtype=torch.int64, device="cuda")
+        pgg.pgg_sweep(full, fmt, L, r, K, seed, pgg.ORDER_IID, 0, n, cnt)
+        torch.cuda.synchronize()
+        row0, n_rows = slab_rows(L, world, rank, pgg_slab_step_rows(fmt, L))
+        good = torch.tensor([int(torch.equal(mine, full[row0:row0 + n_rows]) and torch.equal(counts, cnt))],
+                            device="cuda" if world > 1 else "cpu")
+        dist.all_reduce(good, op=dist.ReduceOp.MIN)
+        ok = bool(good.item())
+    if rank == 0:
+        print(json.dumps({"metric": "elementary strategy updates/sec, one lattice in row slabs", "value": L * L * n / (ms.item() * 1e-3),
+                          "unit": "updates/s", "n_gpus": world, "L": L, "fmt": args.fmt, "mcs": n, "ms": ms.item(),
+                          "us_per_phase": ms.item() * 1e3 / (16 * n), "scaling": "strong", "final_rho_C": counts[-1].item() / L**2,
+                          "equals_unsharded_pgg_sweep": ok, "note": "includes slab set-up, the handle exchange and the final all-reduce"}))
+    dist.barrier()
+    dist.destroy_process_group()
+    if ok is False:
+        raise SystemExit("slabs differ from the unsharded sweep")
+
+
+def main(argv=None) -> None:
+    import argparse
+    ap = argparse.ArgumentParser(description="row slabs of one lattice (DESIGN.md section 10): with no arguments the timing "
+                                 "table of the slab kernel on one device; --sharded under torchrun: one lattice over all ranks")
+    ap.add_argument("--sharded", action="store_true")
+    ap.add_argument("--L", type=int, default=16384)
+    ap.add_argument("--fmt", choices=("bits", "u8"), default="bits")
+    ap.add_argument("--mcs", type=int, default=100)
+    ap.add_argument("--r", type=float, default=3.8)
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--check", action="store_true")
+    args = ap.parse_args(argv)
+    if args.sharded:
+        _run_sharded(args)
+    else:
+        _time_table()
+
+
 if __name__ == "__main__":
-    _time_table()
+    main()

@@ -229,3 +229,22 @@ def test_ipc_handle_opens_in_a_second_process():
         assert np.array_equal(mine.cpu().numpy(), orc.init(L, 0.5, 4242))
     finally:
         pgg.pgg_slab_free(p)
+
+
+def test_sharded_driver_world_size_one():
+    """The one-process-per-GPU driver (slab.run_distributed behind ``python -m paper_1704_08098_b200.slab --sharded``)
+    with the one rank there is: its slab is the whole lattice and its own neighbour, so the handle exchange, the
+    wiring, the chunked calls with running epochs and the final all-reduce all run -- only the IPC mapping does not
+    (test_ipc_handle_opens_in_a_second_process).  --check compares with the unsharded pgg_sweep; the rho_C it prints
+    is compared with the oracle here."""
+    import json
+    L, n = 1024, 5
+    out = subprocess.run([sys.executable, "-m", "paper_1704_08098_b200.slab", "--sharded", "--L", str(L), "--mcs", str(n),
+                          "--fmt", "bits", "--seed", "3", "--check"], capture_output=True, text=True, timeout=600, cwd=ROOT,
+                         env={**__import__("os").environ, "MASTER_PORT": str(36500 + __import__("os").getpid() % 2000)})
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
+    assert d["equals_unsharded_pgg_sweep"] is True and d["n_gpus"] == 1 and d["value"] > 0
+    ref = orc.init(L, 0.5, 3)
+    ref_counts, _ = orc.sweep(ref, 3.8, K, 3, orc.ORDER_IID, 0, n, n_threads=orc.max_threads())
+    assert d["final_rho_C"] == int(ref_counts[-1]) / L**2
