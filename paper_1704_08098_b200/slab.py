@@ -129,9 +129,10 @@ def phase_chunks(t_begin: int, n_mcs: int):
 
 
 class LocalSlabs:
-    """S slabs of one lattice on ONE device.  ``lockstep=True`` launches phase by phase over the slabs (every slab
-    runs phase p before any runs p + 1), with or without the flag protocol; the result equals pgg_sweep on the
-    whole lattice bit for bit."""
+    """S slabs of one lattice on ONE device, launched phase by phase over the slabs on one stream (every slab runs
+    phase p before any runs p + 1, so no kernel ever waits for a later one), with or without the flag protocol;
+    the result equals pgg_sweep on the whole lattice bit for bit.  ``align``: row granularity of the split
+    (None: pgg_slab_step_rows, what the fast kernel wants; 4: any split, general kernels where needed)."""
 
     def __init__(self, full, fmt: int, L: int, n_slabs: int, use_flags: bool = True, align: int | None = None):
         self.fmt, self.L, self.S, self.use_flags = fmt, L, n_slabs, use_flags
