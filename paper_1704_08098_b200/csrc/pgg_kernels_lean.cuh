@@ -200,10 +200,12 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
         eoff[4] = 1;   eoff[5] = 1;  eoff[6] = ps; eoff[7] = ps;
     }
     __syncthreads();
-    if (!PERSIST) asm volatile("griddepcontrol.wait;" ::: "memory");
     // the first / last band waits until the upper / lower neighbour slab has completed the previous phase (its pushes
-    // are in my halo rows, its reads of its own halo copy are over); the other bands touch no halo row
+    // are in my halo rows, its reads of its own halo copy are over); the other bands touch no halo row.  In front of
+    // griddepcontrol.wait: the flags are the neighbours' business, not the previous launch's, so the acquire's
+    // latency overlaps the tail of this slab's previous phase
     if (SLAB) slab_wait_edge(*sl, epoch, blockIdx.x == 0, blockIdx.x == gridDim.x - 1);
+    if (!PERSIST) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t cls = a.order[((size_t)b * a.order_stride + (m % a.order_stride)) * 16 + k];
     const int ci = (int)(cls >> 2), cj = (int)(cls & 3u);
 
