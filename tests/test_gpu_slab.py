@@ -142,6 +142,28 @@ def test_lean_slab_structured_state_and_ragged_split_falls_back():
             assert np.array_equal(got, ref) and np.array_equal(counts, ref_counts)
 
 
+@pytest.mark.parametrize("case", range(10))
+def test_random_splits(case):
+    """Seeded random (L, layout, number of slabs, split granularity, order, start MCS, state): whatever the split and
+    whichever kernel each slab gets, the slabs together are the unsharded oracle."""
+    rng = np.random.default_rng(1000 + case)
+    L = int(rng.choice([32, 64, 128, 160, 256, 1024, 2048]))
+    fmt = int(rng.choice(FMTS)) if L % 32 == 0 else pgg.FMT_U8
+    S = int(rng.integers(1, min(9, L // 4) + 1))
+    align = [None, 4][int(rng.integers(0, 2))]
+    order = [pgg.ORDER_IID, pgg.ORDER_PERM][int(rng.integers(0, 2))]
+    t0 = int(rng.choice([0, 3, 4095, 99_990, 2**32 - 8]))
+    r = float(rng.choice([3.6, 3.8, 4.0, 4.6, 5.5]))
+    seed = int(rng.integers(1, 2**63))
+    lat0 = wl.random_lattice(L, float(rng.choice([0.1, 0.5, 0.9])), case) if rng.integers(0, 3) else wl.blobs_lattice(L, case)
+    n_mcs = 2
+    ref = lat0.copy()
+    ref_counts, _ = orc.sweep(ref, r, K, seed, order, t0, n_mcs, n_threads=orc.max_threads())
+    got, counts, _ = run_slabs(lat0, fmt, S, r, seed, order, t0, n_mcs, use_flags=bool(rng.integers(0, 2)), align=align)
+    assert np.array_equal(got, ref), (L, fmt, S, align, order, t0, r)
+    assert np.array_equal(counts, ref_counts)
+
+
 def test_one_call_for_many_phases_on_a_single_slab():
     """A single slab is its own neighbour both ways, so ONE call may run all phases of several MCS (the way
     run_distributed calls it): mid-MCS start, flags on, against the oracle."""
