@@ -281,6 +281,13 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
                        uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
                        void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,
                        uint32_t epoch0, uint64_t* d_deltas, void* stream);
+/* The prisoner's dilemma (readings G1-G4 above, pgg_pd_sweep) on a row slab: pgg_slab_sweep with the payoffs
+ * (R, S, T, P) in place of r -- same buffer, halo push, flags, kernels (LEAN's ring kernel or the general ones with the
+ * game's table index), errors; the slabs together evolve bit for bit as pgg_pd_sweep evolves the unsharded lattice. */
+int32_t pgg_pd_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double R, double S, double T,
+                          double P, double K, uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin,
+                          uint32_t n_phases, void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag,
+                          uint32_t* d_dn_flag, uint32_t epoch0, uint64_t* d_deltas, void* stream);
 int32_t pgg_slab_alloc(uint64_t bytes, void** d_out);
 int32_t pgg_slab_free(void* d_ptr);
 int32_t pgg_slab_ipc_export(void* d_ptr, uint8_t* h_handle64);

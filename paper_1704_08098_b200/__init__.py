@@ -48,6 +48,9 @@ SIGNATURES = {
     "pgg_slab_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_double, C.c_double,
                                    C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p,
                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]),
+    "pgg_pd_slab_sweep": (C.c_int32, [C.c_void_p, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32] + [C.c_double] * 5 +
+                          [C.c_uint64, C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p,
+                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]),
     "pgg_slab_alloc": (C.c_int32, [C.c_uint64, C.POINTER(C.c_void_p)]),
     "pgg_slab_free": (C.c_int32, [C.c_void_p]),
     "pgg_slab_ipc_export": (C.c_int32, [C.c_void_p, _u8p]),
@@ -179,6 +182,15 @@ def pgg_slab_sweep(d_slab, fmt: int, L: int, row0: int, n_rows: int, r: float, K
     _check(lib().pgg_slab_sweep(_ptr(d_slab), fmt, L, row0, n_rows, r, K, seed, order_mode, t_begin, k_begin, n_phases,
                                 _ptr(d_up_halo), _ptr(d_dn_halo), _ptr(d_flags), _ptr(d_up_flag), _ptr(d_dn_flag),
                                 epoch0, _ptr(d_deltas), _stream(stream)))
+
+
+def pgg_pd_slab_sweep(d_slab, fmt: int, L: int, row0: int, n_rows: int, R: float, S: float, T: float, P: float, K: float,
+                      seed: int, order_mode: int, t_begin: int, k_begin: int, n_phases: int, d_up_halo, d_dn_halo,
+                      d_flags=None, d_up_flag=None, d_dn_flag=None, epoch0: int = 0, d_deltas=None, stream=None) -> None:
+    """pgg_slab_sweep for the prisoner's dilemma: payoffs (R, S, T, P) in place of r."""
+    _check(lib().pgg_pd_slab_sweep(_ptr(d_slab), fmt, L, row0, n_rows, R, S, T, P, K, seed, order_mode, t_begin, k_begin,
+                                   n_phases, _ptr(d_up_halo), _ptr(d_dn_halo), _ptr(d_flags), _ptr(d_up_flag),
+                                   _ptr(d_dn_flag), epoch0, _ptr(d_deltas), _stream(stream)))
 
 
 def pgg_slab_alloc(n_bytes: int) -> int:

@@ -820,11 +820,14 @@ uint32_t pgg_slab_step_rows(int32_t fmt, uint32_t L)
     return 4 * p.R;
 }
 
-int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
-                       uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
-                       void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,
-                       uint32_t epoch0, uint64_t* d_deltas, void* stream_)
+// game = pgg::kGamePGG: pay[0] = r.  game = pgg::kGamePD: pay = {R, S, T, P}.
+static int32_t run_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, int game, const double* pay,
+                              double K, uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
+                              void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,
+                              uint32_t epoch0, uint64_t* d_deltas, void* stream_)
 {
+    const bool pd = game == pgg::kGamePD;
+    const double r = pay[0];
     int32_t rc = check_lattice_args(d_slab, fmt, L);
     if (rc != PGG_OK) return rc;
     if (d_up_halo == nullptr || d_dn_halo == nullptr) return fail(PGG_ERR_NULL, "halo pointer is NULL");
@@ -837,7 +840,8 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     if (order_mode != PGG_ORDER_IID && order_mode != PGG_ORDER_PERM)
         return fail(PGG_ERR_UNSUPPORTED, "slabs run the 16-sublattice schedule only (PGG_ORDER_IID / PGG_ORDER_PERM), not order_mode %d", order_mode);
     if (!(K > 0.0) || !std::isfinite(K)) return fail(PGG_ERR_BAD_PARAM, "K must be finite and > 0");
-    if (!std::isfinite(r)) return fail(PGG_ERR_BAD_PARAM, "r is not finite");
+    for (int q = 0; q < (pd ? 4 : 1); ++q)
+        if (!std::isfinite(pay[q])) return fail(PGG_ERR_BAD_PARAM, pd ? "a payoff (R, S, T, P) is not finite" : "r is not finite");
     if (k_begin >= 16) return fail(PGG_ERR_BAD_PARAM, "k_begin = %u: a MCS has phases 0 .. 15", k_begin);
     if (d_flags != nullptr && (d_up_flag == nullptr || d_dn_flag == nullptr))
         return fail(PGG_ERR_NULL, "d_flags given without both neighbour flag pointers");
@@ -849,8 +853,8 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     if ((unsigned long long)epoch0 + n_phases > 4294967295ull) return fail(PGG_ERR_BAD_PARAM, "epoch0 + n_phases exceeds 2^32 - 1");
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
 
-    uint32_t h_table[pgg::kTableSize];
-    rc = pgg_build_accept_table(r, K, h_table);
+    uint32_t h_table[pgg::kTableSize] = {};
+    rc = pd ? pgg_pd_build_accept_table(pay[0], pay[1], pay[2], pay[3], K, h_table) : pgg_build_accept_table(r, K, h_table);
     if (rc != PGG_OK) return rc;
     Scratch tmp(stream);
     uint64_t* d_seed = nullptr;
@@ -906,14 +910,37 @@ int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uin
     for (uint32_t p = 0; p < n_phases; ++p) {
         const uint32_t q = k_begin + p, t = t_begin + (q >> 4), k = q & 15u;
         if (lean)
-            pgg::lean_slab_launch(lplan, fmt, pa, t - t_begin, k, a, epoch0 + p, stream);
+            pgg::lean_slab_launch(lplan, fmt, pa, t - t_begin, k, a, epoch0 + p, stream, game);
+        else if (fmt == PGG_FMT_U8 && pd)
+            pgg::phase_slab_kernel<pgg::kFmtU8, pgg::kGamePD><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         else if (fmt == PGG_FMT_U8)
             pgg::phase_slab_kernel<pgg::kFmtU8><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
+        else if (pd)
+            pgg::phase_slab_words_kernel<pgg::kGamePD><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         else
-            pgg::phase_slab_words_kernel<<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
+            pgg::phase_slab_words_kernel<pgg::kGamePGG><<<grid, 256, 0, stream>>>(a, t, k, epoch0 + p);
         PGG_LAUNCHED();
     }
     return PGG_OK;
+}
+
+int32_t pgg_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double r, double K,
+                       uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin, uint32_t n_phases,
+                       void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag, uint32_t* d_dn_flag,
+                       uint32_t epoch0, uint64_t* d_deltas, void* stream)
+{
+    return run_slab_sweep(d_slab, fmt, L, row0, n_rows, pgg::kGamePGG, &r, K, seed, order_mode, t_begin, k_begin, n_phases,
+                          d_up_halo, d_dn_halo, d_flags, d_up_flag, d_dn_flag, epoch0, d_deltas, stream);
+}
+
+int32_t pgg_pd_slab_sweep(void* d_slab, int32_t fmt, uint32_t L, uint32_t row0, uint32_t n_rows, double R, double S, double T,
+                          double P, double K, uint64_t seed, int32_t order_mode, uint32_t t_begin, uint32_t k_begin,
+                          uint32_t n_phases, void* d_up_halo, void* d_dn_halo, uint32_t* d_flags, uint32_t* d_up_flag,
+                          uint32_t* d_dn_flag, uint32_t epoch0, uint64_t* d_deltas, void* stream)
+{
+    const double pay[4] = {R, S, T, P};
+    return run_slab_sweep(d_slab, fmt, L, row0, n_rows, pgg::kGamePD, pay, K, seed, order_mode, t_begin, k_begin, n_phases,
+                          d_up_halo, d_dn_halo, d_flags, d_up_flag, d_dn_flag, epoch0, d_deltas, stream);
 }
 
 int32_t pgg_slab_alloc(uint64_t bytes, void** d_out)

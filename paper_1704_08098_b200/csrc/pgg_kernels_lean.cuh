@@ -520,11 +520,11 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
 }
 
 // One phase on a row slab (pgg_slab_sweep): LEAN's kernel on the slab's buffer, rows of layout SRC.
-template <int SRC>
+template <int SRC, int GAME = kGamePGG>
 __global__ void __launch_bounds__(SRC == kFmtU8 ? kLeanThreadsU8 : kLeanThreads, 1)
 phase_lean_slab_kernel(PhaseArgs a, uint32_t m, uint32_t k, LeanPlan g, SlabArgs sa, uint32_t epoch)
 {
-    lean_phase<SRC, kGamePGG, false, true>(a, m, k, g, true, &sa, epoch);
+    lean_phase<SRC, GAME, false, true>(a, m, k, g, true, &sa, epoch);
 }
 
 template <int SRC, int GAME = kGamePGG>
@@ -753,9 +753,11 @@ inline int lean_plan_slab(int fmt, uint32_t L, uint32_t row0, uint32_t n_rows, L
     int rc = lean_plan(fmt, L, 1, p);
     if (rc != 0) return rc;
     if ((n_rows / 4) % p->R != 0 || (row0 / 4) % p->R != 0) return -1;
-    const void* fn = fmt == kFmtU8 ? (const void*)phase_lean_slab_kernel<kFmtU8> : (const void*)phase_lean_slab_kernel<kFmtBits>;
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes);
-    if (e != cudaSuccess) return (int)e;
+    const void* fns[4] = {(const void*)phase_lean_slab_kernel<kFmtU8>, (const void*)phase_lean_slab_kernel<kFmtBits>,
+                          (const void*)phase_lean_slab_kernel<kFmtU8, kGamePD>, (const void*)phase_lean_slab_kernel<kFmtBits, kGamePD>};
+    cudaError_t e = cudaSuccess;
+    for (const void* fn : fns)
+        if ((e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_bytes)) != cudaSuccess) return (int)e;
     int dev = 0, sms = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return (int)e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return (int)e;
@@ -766,7 +768,7 @@ inline int lean_plan_slab(int fmt, uint32_t L, uint32_t row0, uint32_t n_rows, L
 }
 
 inline void lean_slab_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uint32_t m, uint32_t k, const SlabArgs& sa,
-                             uint32_t epoch, cudaStream_t stream)
+                             uint32_t epoch, cudaStream_t stream, int game = kGamePGG)
 {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(p.nb, 1);
@@ -778,7 +780,12 @@ inline void lean_slab_launch(const LeanPlan& p, int fmt, const PhaseArgs& a, uin
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (fmt == kFmtU8)
+    if (game == kGamePD) {
+        if (fmt == kFmtU8)
+            cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel<kFmtU8, kGamePD>, a, m, k, p, sa, epoch);
+        else
+            cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel<kFmtBits, kGamePD>, a, m, k, p, sa, epoch);
+    } else if (fmt == kFmtU8)
         cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel<kFmtU8>, a, m, k, p, sa, epoch);
     else
         cudaLaunchKernelEx(&cfg, phase_lean_slab_kernel<kFmtBits>, a, m, k, p, sa, epoch);

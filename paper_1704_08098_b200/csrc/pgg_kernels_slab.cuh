@@ -159,16 +159,18 @@ __device__ __forceinline__ void slab_finish(const SlabArgs& a, int delta, uint32
     }
 }
 
-// a5-a7 for a site x = (buffer row q, column j) whose drawn neighbour differs: payoff difference, threshold
-// compare, write with the halo push.  Returns the change of the cooperator count.
-template <int FMT>
+// a5-a7 for a site x = (buffer row q, column j) whose drawn neighbour differs: payoff difference (public goods game)
+// or the neighbour counts of x and y (prisoner's dilemma; nx = cooperators among x's four neighbours),
+// threshold compare, write with the halo push.  Returns the change of the cooperator count.
+template <int FMT, int GAME>
 __device__ __forceinline__ int slab_accept(const SlabArgs& a, const SlabLattice<FMT>& lat, int q, int j, int dir, int sx,
-                                           int sy, uint32_t u)
+                                           int sy, int nx, uint32_t u)
 {
     const int L = lat.L, n_rows = (int)a.n_rows, own = q - 3;
     const int yq = q + (dir == 0 ? -1 : dir == 1 ? 1 : 0);
     const int yj = j + (dir == 2 ? -1 : dir == 3 ? 1 : 0);
-    const int idx_t = table_index(payoff_A(lat, q, j) - payoff_A(lat, yq, yj), sx - sy);
+    const int idx_t = GAME == kGamePD ? sx * 25 + nx * 5 + pd_neighbour_count(lat, yq, yj)
+                                      : table_index(payoff_A(lat, q, j) - payoff_A(lat, yq, yj), sx - sy);
     if (u >= a.table[idx_t]) return 0;
     SlabLattice<FMT>::set(a.slab, L, q, j, sy);
     if (own < 3) SlabLattice<FMT>::set(a.up_halo, L, own, j, sy);
@@ -178,7 +180,7 @@ __device__ __forceinline__ int slab_accept(const SlabArgs& a, const SlabLattice<
 
 // uint8 slabs: one thread per active site (V0's step).  A fixed grid strides over the sites, so the flag
 // protocol costs one wait and one post per CTA whatever the slab's size.
-template <int FMT>
+template <int FMT, int GAME = kGamePGG>
 __global__ void __launch_bounds__(256)
 phase_slab_kernel(SlabArgs a, uint32_t t, uint32_t k, uint32_t epoch)
 {
@@ -198,12 +200,13 @@ phase_slab_kernel(SlabArgs a, uint32_t t, uint32_t k, uint32_t epoch)
         const int sx = lat.get(q, j);
         const int s_up = lat.get(q - 1, j), s_dn = lat.get(q + 1, j);
         const int s_lf = lat.get(q, j - 1), s_rt = lat.get(q, j + 1);
-        if (s_up + s_dn + s_lf + s_rt != 4 * sx) {  // S9
+        const int nx = s_up + s_dn + s_lf + s_rt;
+        if (nx != 4 * sx) {  // S9
             uint32_t x0, u;
             step_draw(sk, gi * (uint32_t)L + (uint32_t)j, x0, u);
             const int dir = (int)(x0 >> 30);  // 0:(i-1,j) 1:(i+1,j) 2:(i,j-1) 3:(i,j+1)
             const int sy = dir == 0 ? s_up : dir == 1 ? s_dn : dir == 2 ? s_lf : s_rt;
-            if (sy != sx) delta += slab_accept<FMT>(a, lat, q, j, dir, sx, sy, u);
+            if (sy != sx) delta += slab_accept<FMT, GAME>(a, lat, q, j, dir, sx, sy, nx, u);
         }
     }
     slab_finish(a, delta, t, epoch);
@@ -214,6 +217,7 @@ phase_slab_kernel(SlabArgs a, uint32_t t, uint32_t k, uint32_t epoch)
 // scan of the LEAN kernel, on global memory); the thread then walks those sites.  Later sites of the word
 // see nothing of the earlier ones' flips: they are of the same class, and a step reads no site of the
 // active class but its own.
+template <int GAME = kGamePGG>
 __global__ void __launch_bounds__(256)
 phase_slab_words_kernel(SlabArgs a, uint32_t t, uint32_t k, uint32_t epoch)
 {
@@ -244,7 +248,8 @@ phase_slab_words_kernel(SlabArgs a, uint32_t t, uint32_t k, uint32_t epoch)
             const int dir = (int)(x0 >> 30);
             const uint32_t ny = dir == 0 ? up : dir == 1 ? dn : dir == 2 ? lf : rt;
             const int sx = (int)((c >> p) & 1u), sy = (int)((ny >> p) & 1u);
-            if (sy != sx) delta += slab_accept<kFmtBits>(a, lat, q, 32 * kw + p, dir, sx, sy, u);
+            const int n4 = (int)(((up >> p) & 1u) + ((dn >> p) & 1u) + ((lf >> p) & 1u) + ((rt >> p) & 1u));
+            if (sy != sx) delta += slab_accept<kFmtBits, GAME>(a, lat, q, 32 * kw + p, dir, sx, sy, n4, u);
         }
     }
     slab_finish(a, delta, t, epoch);

@@ -15,7 +15,7 @@ driver; its wiring is covered on CPU with gloo (tests/test_slab_host.py).
 """
 from __future__ import annotations
 
-from . import (FMT_BITS, FMT_U8, SLAB_MAX_MCS, pgg_slab_alloc, pgg_slab_bytes, pgg_slab_free, pgg_slab_ipc_close,
+from . import (FMT_BITS, FMT_U8, SLAB_MAX_MCS, pgg_pd_slab_sweep, pgg_slab_alloc, pgg_slab_bytes, pgg_slab_free, pgg_slab_ipc_close,
                pgg_slab_ipc_export, pgg_slab_ipc_open, pgg_slab_step_rows, pgg_slab_sweep)
 
 HALO = 3          # rows: the read stencil of an elementary step has radius 3
@@ -149,8 +149,9 @@ class LocalSlabs:
             self.wiring.append(wire(sb.ptr, sb.n_rows, up.ptr, up.n_rows, dn.ptr, dn.n_rows, fmt, L))
         self.epoch = 0
 
-    def sweep(self, r: float, K: float, seed: int, order_mode: int, t_begin: int, n_mcs: int, stream=None):
-        """-> int64 tensor [n_mcs]: flips per MCS summed over the slabs (add the running sum to the initial count)."""
+    def sweep(self, r, K: float, seed: int, order_mode: int, t_begin: int, n_mcs: int, stream=None):
+        """-> int64 tensor [n_mcs]: flips per MCS summed over the slabs (add the running sum to the initial count).
+        r: the synergy factor, or a 4-tuple (R, S, T, P) for the prisoner's dilemma (pgg_pd_slab_sweep)."""
         import torch
         dev = self.slabs[0].bytes.device
         deltas = torch.zeros((self.S, max(n_mcs, 1)), dtype=torch.int64, device=dev)
@@ -158,9 +159,14 @@ class LocalSlabs:
             for k in range(16):
                 for rank, (sb, w) in enumerate(zip(self.slabs, self.wiring)):
                     flags = dict(d_flags=w["d_flags"], d_up_flag=w["d_up_flag"], d_dn_flag=w["d_dn_flag"]) if self.use_flags else {}
-                    pgg_slab_sweep(sb.ptr, self.fmt, self.L, sb.row0, sb.n_rows, r, K, seed, order_mode, t, k, 1,
-                                   w["d_up_halo"], w["d_dn_halo"], epoch0=self.epoch,
-                                   d_deltas=deltas[rank, t - t_begin:], stream=stream, **flags)
+                    if isinstance(r, (tuple, list)):
+                        pgg_pd_slab_sweep(sb.ptr, self.fmt, self.L, sb.row0, sb.n_rows, *r, K, seed, order_mode, t, k, 1,
+                                          w["d_up_halo"], w["d_dn_halo"], epoch0=self.epoch,
+                                          d_deltas=deltas[rank, t - t_begin:], stream=stream, **flags)
+                    else:
+                        pgg_slab_sweep(sb.ptr, self.fmt, self.L, sb.row0, sb.n_rows, r, K, seed, order_mode, t, k, 1,
+                                       w["d_up_halo"], w["d_dn_halo"], epoch0=self.epoch,
+                                       d_deltas=deltas[rank, t - t_begin:], stream=stream, **flags)
                 self.epoch += 1
         return deltas[:, :n_mcs].sum(dim=0)
 

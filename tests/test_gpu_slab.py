@@ -164,6 +164,23 @@ def test_random_splits(case):
     assert np.array_equal(counts, ref_counts)
 
 
+@pytest.mark.parametrize("fmt", FMTS)
+@pytest.mark.parametrize("L,S,align", [(64, 3, None), (96, 2, None), (1024, 4, None), (1024, 3, 4), (2048, 2, None)])
+def test_prisoners_dilemma_on_slabs(fmt, L, S, align):
+    """The second game (pgg_pd_sweep) on row slabs: general kernels (L = 64, 96, the ragged split of
+    1024) and LEAN on the slab (1024, 2048), against the unsharded prisoner's-dilemma oracle."""
+    if fmt == pgg.FMT_BITS and L % 32:
+        pytest.skip("bit rows need L % 32 == 0")
+    pay, n_mcs, seed = (1.0, 0.0, 1.3, 0.1), 4, 77
+    lat0 = wl.random_lattice(L, 0.5, 23)
+    ref = lat0.copy()
+    ref_counts = orc.pd_sweep(ref, *pay, K, seed, orc.ORDER_IID, 3, n_mcs)
+    got, counts, _ = run_slabs(lat0, fmt, S, pay, seed, pgg.ORDER_IID, 3, n_mcs, use_flags=True, align=align)
+    assert pgg.pgg_get_variant_used() == (pgg.VARIANT_LEAN if L >= 1024 and align is None else pgg.VARIANT_V0)
+    assert np.array_equal(got, ref), f"{int((got != ref).sum())} sites differ"
+    assert np.array_equal(counts, ref_counts)
+
+
 def test_one_call_for_many_phases_on_a_single_slab():
     """A single slab is its own neighbour both ways, so ONE call may run all phases of several MCS (the way
     run_distributed calls it): mid-MCS start, flags on, against the oracle."""
