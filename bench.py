@@ -372,7 +372,7 @@ def run_ours(args):
     except (ValueError, OSError):
         pass
     if (fmt == pgg.FMT_BITS or packed) and not dtile:
-        # the packed lattice is L2-resident: its bound is the integer pipes, not HBM
+        # the packed lattice is L2-resident: its bound is integer instruction issue, not HBM
         alu.update({"traffic": roofline["traffic"], "kernel": roofline["kernel"], "avg_launch_us": phase_us,
                     "hbm_context": {k: roofline[k] for k in ("achieved", "peak", "frac", "algorithmic_bytes_per_launch")}})
         if packed:
