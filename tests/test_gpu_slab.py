@@ -287,3 +287,16 @@ def test_sharded_driver_world_size_one():
     ref = orc.init(L, 0.5, 3)
     ref_counts, _ = orc.sweep(ref, 3.8, K, 3, orc.ORDER_IID, 0, n, n_threads=orc.max_threads())
     assert d["final_rho_C"] == int(ref_counts[-1]) / L**2
+
+
+def test_sharded_driver_long_run_crosses_the_call_limit():
+    """4200 MCS = 67 200 phases through run_distributed at world size 1: two calls (4096 + 104 MCS, PGG_SLAB_MAX_MCS),
+    epochs running on from the first into the second, against the unsharded pgg_sweep (--check; that path's own
+    run across the 4096-MCS boundary is checked against the oracle in test_gpu_parity.py)."""
+    import json
+    out = subprocess.run([sys.executable, "-m", "paper_1704_08098_b200.slab", "--sharded", "--L", "1024", "--mcs", "4200",
+                          "--fmt", "bits", "--seed", "9", "--r", "3.9", "--check"], capture_output=True, text=True, timeout=900,
+                         cwd=ROOT, env={**__import__("os").environ, "MASTER_PORT": str(38500 + __import__("os").getpid() % 2000)})
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
+    assert d["equals_unsharded_pgg_sweep"] is True and d["mcs"] == 4200
