@@ -57,7 +57,7 @@ constexpr int kLeanConsumers = 16;
 constexpr int kLeanPackers = 4;   // uint8 source: warps that turn staged bytes into ring bits
 constexpr int kLeanThreads = (kLeanConsumers + 1) * 32;                    // bit-packed source
 constexpr int kLeanThreadsU8 = (kLeanConsumers + 1 + kLeanPackers) * 32;   // uint8 source
-constexpr int kLeanQ1Cap = 160;   // 8-byte entries per warp: leftover (< 32) + at most 128 per extraction round
+constexpr int kLeanQ1Cap = 192;   // 8-byte entries per warp: leftover (< 64) + at most 128 per extraction round
 constexpr int kLeanQ2Cap = 64;    // 16-byte entries per warp (a ring: power of two)
 constexpr int kLeanWarpQBytes = kLeanQ1Cap * 8 + kLeanQ2Cap * 16;
 constexpr int kLeanMaxSlots = 12; // staging slots (uint8) / ring chunks (bit-packed): barrier array size
@@ -411,7 +411,7 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
         // full batches from the front of Q1, two at a time while 64 wait (two independent Philox
         // chains); the leftover (< 32) moves to the front
         auto run_batches = [&]() {
-            if (n1 < 32u) return;
+            if (n1 < 64u) return;
             uint32_t head = 0;
             while (n1 - head >= 64u) {
                 uint4 wa, wb;
@@ -421,15 +421,13 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
                 push2(gb, wb);
                 head += 64u;
             }
-            if (n1 - head >= 32u) {
-                run_level1(head, 32u);
-                head += 32u;
-            }
-            const uint32_t left = n1 - head;
-            uint2 e = make_uint2(0u, 0u);
-            if ((uint32_t)lane < left) e = q1[head + lane];
+            const uint32_t left = n1 - head;  // < 64: waits for the next round, so that every batch runs in a pair
+            uint2 e0 = make_uint2(0u, 0u), e1 = make_uint2(0u, 0u);
+            if ((uint32_t)lane < left) e0 = q1[head + lane];
+            if ((uint32_t)lane + 32u < left) e1 = q1[head + 32 + lane];
             __syncwarp();
-            if ((uint32_t)lane < left) q1[lane] = e;
+            if ((uint32_t)lane < left) q1[lane] = e0;
+            if ((uint32_t)lane + 32u < left) q1[32 + lane] = e1;
             __syncwarp();
             n1 = left;
         };
@@ -459,7 +457,11 @@ __device__ __forceinline__ void lean_phase(const PhaseArgs& a, uint32_t m, uint3
             return true;
         };
         auto drain_all = [&]() {
-            if (n1) {  // < 32
+            if (n1 > 32u) {  // < 64
+                run_level1(0u, 32u);
+                run_level1(32u, n1 - 32u);
+                n1 = 0;
+            } else if (n1) {
                 run_level1(0u, n1);
                 n1 = 0;
             }
