@@ -233,8 +233,8 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
             if ((uint32_t)lane < cnt) go = level1(q1[head + lane], w);
             push2(go, w);
         };
-        auto run_batches = [&]() {
-            if (n1 < 32u) return;
+        auto run_batches = [&]() {  // every batch in an interleaved pair; up to 63 entries wait (as in LEAN)
+            if (n1 < 64u) return;
             uint32_t head = 0;
             while (n1 - head >= 64u) {
                 uint4 wa, wb;
@@ -244,15 +244,13 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
                 push2(gb, wb);
                 head += 64u;
             }
-            if (n1 - head >= 32u) {
-                run_level1(head, 32u);
-                head += 32u;
-            }
             const uint32_t left = n1 - head;
-            uint2 e = make_uint2(0u, 0u);
-            if ((uint32_t)lane < left) e = q1[head + lane];
+            uint2 e0 = make_uint2(0u, 0u), e1 = make_uint2(0u, 0u);
+            if ((uint32_t)lane < left) e0 = q1[head + lane];
+            if ((uint32_t)lane + 32u < left) e1 = q1[head + 32 + lane];
             __syncwarp();
-            if ((uint32_t)lane < left) q1[lane] = e;
+            if ((uint32_t)lane < left) q1[lane] = e0;
+            if ((uint32_t)lane + 32u < left) q1[32 + lane] = e1;
             __syncwarp();
             n1 = left;
         };
@@ -296,7 +294,11 @@ sweep_cluster_kernel(PhaseArgs a, uint32_t m0, uint32_t n_mcs, ClusterPlan g)
                 }
             }
         }
-        if (n1) {  // < 32
+        if (n1 > 32u) {  // < 64
+            run_level1(0u, 32u);
+            run_level1(32u, n1 - 32u);
+            n1 = 0;
+        } else if (n1) {
             run_level1(0u, n1);
             n1 = 0;
         }
